@@ -1,0 +1,166 @@
+/*
+ * qmc_crowd.h -- C ABI of the B200-native crowd move (libqmc_crowd.so).
+ *
+ * One thing is built here: the particle-by-particle electron move of arXiv:2209.14487
+ * applied to a whole crowd of walkers in lock-step.  Citations:
+ *   P:n   = /root/reference/PAPER.md line n
+ *   BJ    = BASELINE.json north_star
+ *   D:Cx / D:Ax = DESIGN.md "Readings" (restated from SURVEY.md 8(c))
+ *
+ *   Alg. 1 lines 5-9: propose, ratio, gradient at the new position, accept/reject.
+ *   Alg. 3 / Alg. 4: every routine serves all walkers of the crowd in
+ *   one batched call and all walkers advance in lock-step for each single particle move.
+ *   a crowd is a sub-population advanced in lock-step; one crowd is the legacy
+ *   single-stream case.  The arithmetic inside each call is named by BJ; the formula each call
+ *   evaluates is given with the call.
+ *
+ * Conventions
+ *   - plain C types only; nothing throws; every call returns a qmc_status (QMC_OK = 0) and the
+ *     text of the last failure on this host thread is kept for qmc_last_error().
+ *   - "DEVICE" pointers are CUDA device pointers of the current device, "HOST" pointers are host
+ *     memory.  BORROWED pointers must outlive the crowd; the library never frees them.
+ *   - the library allocates NO device memory: the caller hands it one workspace
+ *     (size from qmc_crowd_workspace_bytes) and the coefficient table (BJ: "PyTorch only for
+ *     device memory and streams").
+ *   - all step calls are asynchronous on desc.stream unless stated otherwise.
+ *   - N electrons, n = N/2 per spin, M = n orbitals shared by both spins (D:A5), W walkers.
+ *     Electrons [0,n) are spin-up (determinant 0), [n,N) spin-down (determinant 1).
+ *   - there is no CPU fallback anywhere: without a CUDA device every call that touches the
+ *     device fails with QMC_ERR_CUDA.
+ */
+#ifndef QMC_CROWD_H
+#define QMC_CROWD_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qmc_crowd qmc_crowd_t; /* opaque; owned by the library (host struct only) */
+
+typedef enum {
+  QMC_OK = 0,
+  QMC_ERR_INVALID_ARG = 1, /* NULL pointer, bad size, unsupported shape                         */
+  QMC_ERR_CUDA = 2,        /* a CUDA call failed (text in qmc_last_error)                       */
+  QMC_ERR_WORKSPACE = 3,   /* workspace NULL, misaligned (256 B) or too small                   */
+  QMC_ERR_SINGULAR = 4,    /* a Slater matrix had a zero / non-finite pivot (D:A16)             */
+  QMC_ERR_STATE = 5        /* step calls out of order, or a flush the schedule requires is due  */
+} qmc_status;
+
+typedef struct {
+  int32_t n_elec;      /* N, even, >= 2                                                          */
+  int32_t n_orb;       /* M, must equal N/2 (D:A5)                                               */
+  int32_t grid[3];     /* Ng per axis, >= 1                                                      */
+  int32_t coef_dtype;  /* 0 = fp32 table (orbitals evaluated in fp32), 1 = fp64 table            */
+  double box[3];       /* L per axis, orthorhombic periodic cell                                 */
+  const void* coefs;   /* DEVICE, BORROWED: P[gx][gy][gz][orb_stride], orbital index innermost   */
+                       /* (BJ: "coefficients stored orbital-innermost"), 16-byte aligned         */
+  int64_t orb_stride;  /* elements between grid points: >= n_orb, multiple of 4 (fp32) / 2 (fp64)*/
+  double j2_a, j2_b;   /* two-body Jastrow u(r) = a r / (1 + b r)  (D:C3)                        */
+  double tau;          /* time step of the drift-diffusion proposal (D:C4)                       */
+  int32_t n_walkers;   /* W >= 1                                                                 */
+  int32_t walker_id0;  /* global id of walker 0: Philox counter word 0 is walker_id0 + w (D:C7), */
+                       /* so splitting a population into crowds does not change any trajectory   */
+  int32_t delay_rank;  /* 1 = Sherman-Morrison rank-1 (D:C5); 2..64 = delayed rank-k (D:C6)      */
+  int32_t _pad;
+  uint64_t seed;       /* Philox key (lo, hi)                                                    */
+  void* workspace;     /* DEVICE, BORROWED, 256-byte aligned                                     */
+  size_t workspace_bytes; /* >= qmc_crowd_workspace_bytes(&desc)                                 */
+  void* stream;        /* cudaStream_t (0 = legacy default stream), BORROWED                     */
+} qmc_crowd_desc;
+
+/* Bytes of device workspace a crowd of this shape needs (positions, transposed inverses,
+ * per-electron gradient/Laplacian caches, delayed window, per-move scratch). 0 on a bad desc. */
+size_t qmc_crowd_workspace_bytes(const qmc_crowd_desc* desc);
+
+/* BJ "qmc_crowd_create".  Copies pos_dev (DEVICE, [W][N][3] fp64) into the workspace, evaluates
+ * the Slater matrices A^s_ij = phi_j(r_{s n + i}) of both spins with the spline kernel (D:C1,C2),
+ * inverts them on the device by Gauss-Jordan with partial pivoting into the stored form
+ * B = (A^-1)^T (row = electron, D:A9), fills the per-electron caches of grad phi / lap phi
+ * (D:A12, A13), and synchronises the stream.  Returns QMC_ERR_SINGULAR (and no crowd) when a
+ * pivot is zero or not finite. */
+int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crowd_t** out);
+int qmc_crowd_destroy(qmc_crowd_t* crowd);
+
+/* ---- one electron index k for ALL walkers of the crowd (Alg. 3 line 3) -------------
+ * The three calls must be issued in this order for the same k; otherwise QMC_ERR_STATE.
+ * With delay_rank > 1 a flush is due after every delay_rank proposed moves of a spin block
+ * and at the end of each spin block (D:C6 schedule); qmc_spo_vgl returns QMC_ERR_STATE if that
+ * flush was not issued (qmc_sweep does it itself).                                            */
+
+/* BJ "qmc_spo_vgl" = Alg. 1 line 5 (reading D:A1) followed by the orbital evaluation.
+ *  (a) current inverse row b of electron k with the pending delayed window applied (D:C6),
+ *      G_k(R) = b . grad phi(r_k) [cache] + grad_k ln Psi_J(R)   (D:C2, C3, A13);
+ *  (b) if rnew_dev == NULL: Delta = fl32(tau G_k(R) + sqrt(tau) chi), chi from Philox
+ *      counter (walker id, k, sweep, 0), r' = r_k + Delta (D:C4, C7);
+ *      else r' = rnew_dev[w] (DEVICE, [W][3] fp64) and Delta = r' - r_k (teacher forcing);
+ *  (c) phi_j(r'), grad phi_j(r'), lap phi_j(r') for j < M: the 4x4x4 tricubic B-spline stencil
+ *      (D:C1), evaluated in the table's precision.
+ * phi / dphi / d2phi: optional DEVICE outputs (NULL to skip), element type = table type,
+ * compact layouts [W][M], [W][3][M], [W][M].                                                  */
+int qmc_spo_vgl(qmc_crowd_t* crowd, int k, const double* rnew_dev, void* phi, void* dphi, void* d2phi);
+
+/* BJ "qmc_ratio_grad" = Alg. 1 lines 7-8.  rho_D = b . phi(r') (matrix-determinant
+ * lemma, D:C2); rho_J = exp(sum_{i!=k} u(|r'-r_i|) - u(|r_k-r_i|)) (D:C3);
+ * ratio[w] = rho_D rho_J;  grad[w] = (b . grad phi(r'))/rho_D + grad_k ln Psi_J(R').
+ * ratio: DEVICE [W] fp64 or NULL; grad: DEVICE [W][3] fp64 or NULL.                           */
+int qmc_ratio_grad(qmc_crowd_t* crowd, int k, double* ratio, double* grad);
+
+/* BJ "qmc_accept_reject" = Alg. 1 line 9 (reading D:A3).  p = rho^2 exp(logGb - logGf)
+ * with the applied Delta (D:C4); u from Philox counter (walker id, k, sweep, 1); accept <=> u < p,
+ * non-finite p or rho_D == 0 rejects.  On accept: r_k <- r', caches <- new, and the inverse is
+ * updated by Sherman-Morrison (delay_rank 1, D:C5) or the move is appended to the delayed
+ * window (D:C6).  On reject nothing changes.  accepted: DEVICE [W] uint8 or NULL.      */
+int qmc_accept_reject(qmc_crowd_t* crowd, int k, uint8_t* accepted);
+
+/* BJ "qmc_flush_delayed" (D:C6): B <- B0 - (B0 V^T - E) S^-T C for every walker with a
+ * non-empty window (FP64 DMMA), then empties the windows.  No-op for delay_rank 1 or when
+ * nothing was proposed since the last flush.                                                  */
+int qmc_flush_delayed(qmc_crowd_t* crowd);
+
+/* BJ "qmc_sweep": n_sweeps full sweeps k = 0..N-1 (P:73 particle-by-particle; Alg. 3 lines 2-4)
+ * of propose / vgl / ratio / accept with the flush schedule of D:C6; the sweep index (Philox
+ * counter word 2) advances by one per sweep.  Ends flushed.  Asynchronous.                    */
+int qmc_sweep(qmc_crowd_t* crowd, int n_sweeps);
+
+/* Host-buffer form of the same path (bench.py "e2e"): copies pos_host (HOST, [W][N][3] fp64)
+ * to the device, rebuilds Slater matrices / inverses / caches from it (as qmc_crowd_create),
+ * runs n_sweeps sweeps, copies the positions back into pos_host and the three counters
+ * (proposed, accepted, flushes; totals since create) into stats_host[3].  Synchronous.       */
+int qmc_sweep_host(qmc_crowd_t* crowd, double* pos_host, int n_sweeps, uint64_t* stats_host);
+
+/* ---- state access for tests: synchronous copies on desc.stream -------------------------- */
+int qmc_crowd_get_positions(qmc_crowd_t* crowd, double* pos_dev /* DEVICE [W][N][3] */);
+int qmc_crowd_set_positions(qmc_crowd_t* crowd, const double* pos_dev); /* rebuilds, may be SINGULAR */
+/* transposed inverse of one spin, compact DEVICE [W][n][n]; with a window open this is B0 */
+int qmc_crowd_get_inverse(qmc_crowd_t* crowd, int spin, double* binv_dev);
+int qmc_crowd_set_inverse(qmc_crowd_t* crowd, int spin, const double* binv_dev); /* window must be empty */
+/* per-electron caches, element type = table type, compact DEVICE [W][N][3][M] and [W][N][M] */
+int qmc_crowd_get_caches(qmc_crowd_t* crowd, void* dphi_dev, void* d2phi_dev);
+/* delayed window: m[W] int32, rows[W][k] int32, V[W][k][n], C[W][k][n], Sinv[W][k][k] fp64
+ * (k = delay_rank; entries at or beyond m[w] are unspecified); any pointer may be NULL      */
+int qmc_crowd_get_window(qmc_crowd_t* crowd, int32_t* m_dev, int32_t* rows_dev, double* v_dev, double* c_dev,
+                         double* sinv_dev);
+/* everything the last move computed, one entry per walker, DEVICE, any pointer may be NULL:
+ * rnew[W][3], delta[W][3], g_old[W][3], g_new[W][3], rho_d[W], rho_j[W], p[W], u[W] fp64,
+ * brow[W][n] = inverse row used for the move                                               */
+int qmc_crowd_get_move(qmc_crowd_t* crowd, double* rnew, double* delta, double* g_old, double* g_new, double* rho_d,
+                       double* rho_j, double* p, double* u, double* brow);
+int qmc_crowd_set_sweep_index(qmc_crowd_t* crowd, uint32_t s);
+/* totals since create; synchronous */
+int qmc_crowd_stats(qmc_crowd_t* crowd, uint64_t* proposed, uint64_t* accepted, uint64_t* flushes);
+/* kernels + memset nodes this crowd has launched since create (host counter, for bench.py) */
+uint64_t qmc_crowd_launch_count(const qmc_crowd_t* crowd);
+/* option 0 (QMC_OPT_GRAPH): 1 = qmc_sweep replays one captured CUDA graph per sweep (default),
+ * 0 = plain stream launches.                                                                */
+int qmc_crowd_set_option(qmc_crowd_t* crowd, int option, int value);
+#define QMC_OPT_GRAPH 0
+
+const char* qmc_last_error(void); /* thread-local, never NULL */
+const char* qmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,6 @@
+"""B200-native crowd move of arXiv:2209.14487: thin binding over the C-ABI library libqmc_crowd.so.
+
+The product is the CUDA library (csrc/, include/qmc_crowd.h); this package only marshals arguments.
+"""
+from .binding import (Crowd, CrowdDesc, QmcError, EXPORTS, QMC_OPT_GRAPH, QMC_OK, QMC_ERR_INVALID_ARG,  # noqa: F401
+                      QMC_ERR_CUDA, QMC_ERR_WORKSPACE, QMC_ERR_SINGULAR, QMC_ERR_STATE, lib_path, load)

@@ -1,0 +1,125 @@
+// common.cuh -- device-side view of a crowd and small helpers shared by the kernels.
+//
+// Layout of the caller-owned workspace:
+//   R      fp64 [W][N][3]          positions, not wrapped (D:C1)
+//   Binv   fp64 [W][2][ns][ns]     B = (A^-1)^T per spin, row = electron (D:A9); ns = n rounded
+//                                  up to 16, padding rows/columns are zero and stay zero
+//   cache  T    [W][N][4][ns]      d/dx, d/dy, d/dz, laplacian of phi at the electron's current
+//                                  position (D:A12, A13); T = table type
+//   vgl    T    [W][5][ns]         phi, d/dx, d/dy, d/dz, lap at the proposed position
+//   brow   fp64 [W][ns]            inverse row of the moved electron, window applied (D:C6)
+//   V, C   fp64 [W][kdp][ns]       delayed window rows; kdp = delay rank padded to 8/16/32/64
+//   Sinv   fp64 [W][kdp][kdp]      inverse of S = V C^T, grown by bordering
+//   per-walker scalars of the move in flight (rnew, delta, g_old, g_new, ...)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace qmc {
+
+struct CrowdDev {
+  int W, N, n, M, ns;
+  int kd, kdp;
+  int walker_id0;
+  unsigned seed_lo, seed_hi;
+  int grid[3];
+  double tau, sqrt_tau, j2_a, j2_b;
+  double box[3], inv_box[3], inv_h[3];
+  unsigned orb_stride_v;  // orbital stride of the table in 16-byte vectors
+  unsigned tab_vecs;      // vectors of the table that hold orbitals < orb_stride (per grid point)
+  const void* coefs;
+  double* R;
+  double* Binv;
+  void* cache;
+  void* vgl;
+  double* brow;
+  double *rnew, *delta, *g_old, *g_new;      // [W][3]
+  double *usum_old, *rho_d, *rho_j, *p, *u;  // [W]
+  unsigned char* accepted;                   // [W]
+  double *V, *C, *Sinv, *pvec, *yvec;
+  int* rows;                                 // [W][kdp]
+  int* mwin;                                 // [W]
+  unsigned long long* counters;              // [0] accepted moves
+  unsigned* sweep;                           // [1] Philox counter word 2
+  int* status;                               // [1] != 0: singular matrix met
+};
+
+template <typename T> struct Vec16;
+template <> struct Vec16<float> { static constexpr int W = 4; };
+template <> struct Vec16<double> { static constexpr int W = 2; };
+
+__device__ __forceinline__ void ld16(const float* p, float (&v)[4])
+{
+  const float4 q = __ldg(reinterpret_cast<const float4*>(p));
+  v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+}
+__device__ __forceinline__ void ld16(const double* p, double (&v)[2])
+{
+  const double2 q = __ldg(reinterpret_cast<const double2*>(p));
+  v[0] = q.x; v[1] = q.y;
+}
+__device__ __forceinline__ void st16(float* p, const float (&v)[4])
+{
+  *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+}
+__device__ __forceinline__ void st16(double* p, const double (&v)[2])
+{
+  *reinterpret_cast<double2*>(p) = make_double2(v[0], v[1]);
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Sum NV values over a block of NT threads; every thread gets the totals. sm: NV*NT/32 doubles.
+template <int NV, int NT>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* sm)
+{
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) v[i] = warp_sum(v[i]);
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) sm[warp * NV + i] = v[i];
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < NT / 32; ++w) s += sm[w * NV + i];
+    v[i] = s;
+  }
+  __syncthreads();
+}
+
+// ---- Philox4x32-10 (Salmon et al., SC'11; D:C7). Counter (walker id, k, sweep, tag). ----
+__device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0,
+                                              unsigned k1, unsigned (&out)[4])
+{
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    if (r > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+    const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    const unsigned n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+__device__ __forceinline__ double u01(unsigned x) { return ((double)x + 0.5) * (1.0 / 4294967296.0); }
+
+// FP64 tensor-core tile: D(8x8) += A(8x4, row) B(4x8, col). Lane l holds A[l/4][l%4],
+// B[l%4][l/4] and D[l/4][2(l%4) + {0,1}].  SASS: DMMA.8x8x4.
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b)
+{
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c[0]), "+d"(c[1])
+               : "d"(a), "d"(b));
+}
+
+}  // namespace qmc

@@ -1,0 +1,678 @@
+// qmc_crowd.cu -- host side of libqmc_crowd.so: the C ABI of include/qmc_crowd.h.
+// Argument checking, workspace carving, kernel launches and the lock-step sweep schedule
+// (Alg. 3; flush schedule D:C6).  Every step of the path runs in the kernels of
+// spline.cuh / move.cuh / update.cuh / invert.cuh; there is no CPU fallback.
+#include "../../include/qmc_crowd.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "invert.cuh"
+#include "move.cuh"
+#include "spline.cuh"
+#include "update.cuh"
+
+using namespace qmc;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...)
+{
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                              \
+  do {                                                                                              \
+    cudaError_t e_ = (expr);                                                                        \
+    if (e_ != cudaSuccess) return fail(QMC_ERR_CUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+  } while (0)
+
+#define LAUNCH_CHECK(c)                                                                             \
+  do {                                                                                              \
+    ++(c)->launches;                                                                                \
+    cudaError_t e_ = cudaGetLastError();                                                            \
+    if (e_ != cudaSuccess) return fail(QMC_ERR_CUDA, "kernel launch: %s (%s:%d)", cudaGetErrorString(e_), __FILE__, __LINE__); \
+  } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+enum StepState { ST_IDLE = 0, ST_HAVE_VGL = 1, ST_HAVE_RATIO = 2 };
+
+}  // namespace
+
+struct qmc_crowd {
+  qmc_crowd_desc desc;
+  CrowdDev dev;
+  cudaStream_t stream;
+  int is_f64;
+  size_t elem;             // sizeof(table element)
+  int state, state_k;
+  int win_spin;            // spin block of the open window, -1 if none
+  std::vector<int> win_rows;  // electrons (within the spin block) proposed since the last flush
+  uint64_t proposed, flushes, launches;
+  uint32_t sweep_host;
+  int use_graph;
+  cudaGraphExec_t graph_exec;
+  unsigned char* acc_scratch;  // unused output sink
+};
+
+namespace {
+
+int padded_rank(int kd)
+{
+  int p = 8;
+  while (p < kd) p *= 2;
+  return p;
+}
+
+// Carves the workspace; with base == nullptr only measures. Returns total bytes.
+size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
+{
+  const size_t W = (size_t)ds->n_walkers, N = (size_t)ds->n_elec, n = N / 2;
+  const size_t ns = align_up(n, 16);
+  const size_t kdp = (size_t)padded_rank(ds->delay_rank);
+  const size_t el = ds->coef_dtype ? 8 : 4;
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    char* p = base ? base + off : nullptr;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  char* R = take(W * N * 3 * 8);
+  char* Binv = take(W * 2 * ns * ns * 8);
+  char* cache = take(W * N * 4 * ns * el);
+  char* vgl = take(W * 5 * ns * el);
+  char* brow = take(W * ns * 8);
+  char* rnew = take(W * 3 * 8);
+  char* delta = take(W * 3 * 8);
+  char* g_old = take(W * 3 * 8);
+  char* g_new = take(W * 3 * 8);
+  char* usum_old = take(W * 8);
+  char* rho_d = take(W * 8);
+  char* rho_j = take(W * 8);
+  char* p = take(W * 8);
+  char* u = take(W * 8);
+  char* accepted = take(W);
+  char* acc_sink = take(W);
+  char* V = take(ds->delay_rank > 1 ? W * kdp * ns * 8 : 8);
+  char* C = take(ds->delay_rank > 1 ? W * kdp * ns * 8 : 8);
+  char* Sinv = take(ds->delay_rank > 1 ? W * kdp * kdp * 8 : 8);
+  char* pvec = take(W * kdp * 8);
+  char* yvec = take(W * kdp * 8);
+  char* rows = take(W * kdp * 4);
+  char* mwin = take(W * 4);
+  char* counters = take(4 * 8);
+  char* sweep = take(4);
+  char* status = take(4);
+  if (d) {
+    d->R = (double*)R; d->Binv = (double*)Binv; d->cache = cache; d->vgl = vgl; d->brow = (double*)brow;
+    d->rnew = (double*)rnew; d->delta = (double*)delta; d->g_old = (double*)g_old; d->g_new = (double*)g_new;
+    d->usum_old = (double*)usum_old; d->rho_d = (double*)rho_d; d->rho_j = (double*)rho_j;
+    d->p = (double*)p; d->u = (double*)u; d->accepted = (unsigned char*)accepted;
+    d->V = (double*)V; d->C = (double*)C; d->Sinv = (double*)Sinv; d->pvec = (double*)pvec; d->yvec = (double*)yvec;
+    d->rows = (int*)rows; d->mwin = (int*)mwin; d->counters = (unsigned long long*)counters;
+    d->sweep = (unsigned*)sweep; d->status = (int*)status;
+    (void)acc_sink;
+  }
+  return off;
+}
+
+int check_desc(const qmc_crowd_desc* ds)
+{
+  if (!ds) return fail(QMC_ERR_INVALID_ARG, "desc is NULL");
+  if (ds->n_elec < 2 || (ds->n_elec & 1)) return fail(QMC_ERR_INVALID_ARG, "n_elec must be even and >= 2");
+  if (ds->n_orb != ds->n_elec / 2) return fail(QMC_ERR_INVALID_ARG, "n_orb must equal n_elec/2");
+  if (ds->n_walkers < 1) return fail(QMC_ERR_INVALID_ARG, "n_walkers must be >= 1");
+  if (ds->coef_dtype != 0 && ds->coef_dtype != 1) return fail(QMC_ERR_INVALID_ARG, "coef_dtype must be 0 or 1");
+  if (ds->delay_rank < 1 || ds->delay_rank > 64) return fail(QMC_ERR_INVALID_ARG, "delay_rank must be in [1,64]");
+  const int vw = ds->coef_dtype ? 2 : 4;
+  if (ds->orb_stride < ds->n_orb || ds->orb_stride % vw) return fail(QMC_ERR_INVALID_ARG, "orb_stride must be >= n_orb and a multiple of %d", vw);
+  double tab = (double)ds->orb_stride / vw;
+  for (int c = 0; c < 3; ++c) {
+    if (ds->grid[c] < 1) return fail(QMC_ERR_INVALID_ARG, "grid must be >= 1");
+    if (!(ds->box[c] > 0.0) || !std::isfinite(ds->box[c])) return fail(QMC_ERR_INVALID_ARG, "box must be positive");
+    tab *= ds->grid[c];
+  }
+  if (tab >= 4294967296.0) return fail(QMC_ERR_INVALID_ARG, "coefficient table larger than 2^32 16-byte vectors");
+  if (!(ds->tau > 0.0) || !std::isfinite(ds->tau)) return fail(QMC_ERR_INVALID_ARG, "tau must be positive");
+  return QMC_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// launch helpers (all on c->stream)
+// ------------------------------------------------------------------------------------------
+namespace {
+
+template <typename T>
+int launch_build_t(qmc_crowd* c)
+{
+  const CrowdDev& d = c->dev;
+  const size_t chunks = (size_t)d.ns / Vec16<T>::W;
+  const size_t items = (size_t)d.W * d.N * chunks;
+  const size_t blocks = (items + SPLINE_NT - 1) / SPLINE_NT;
+  if (blocks > 0x7fffffffull) return fail(QMC_ERR_INVALID_ARG, "crowd too large for one build launch");
+  spline_build_kernel<T><<<(unsigned)blocks, SPLINE_NT, 0, c->stream>>>(d);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+// spline at all electron positions -> caches + A^T; Gauss-Jordan; status check (synchronises)
+int rebuild(qmc_crowd* c)
+{
+  const CrowdDev& d = c->dev;
+  CUDA_TRY(cudaMemsetAsync(d.Binv, 0, (size_t)d.W * 2 * d.ns * d.ns * 8, c->stream));
+  CUDA_TRY(cudaMemsetAsync(d.mwin, 0, (size_t)d.W * 4, c->stream));
+  CUDA_TRY(cudaMemsetAsync(d.status, 0, 4, c->stream));
+  c->launches += 3;
+  int st = c->is_f64 ? launch_build_t<double>(c) : launch_build_t<float>(c);
+  if (st) return st;
+  const size_t smem = (size_t)(2 * d.ns + 2 * (INV_NT / 32)) * 8 + (size_t)d.ns * 4 + 64;
+  if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  invert_kernel<<<(unsigned)(d.W * 2), INV_NT, smem, c->stream>>>(d);
+  LAUNCH_CHECK(c);
+  int status = 0;
+  CUDA_TRY(cudaMemcpyAsync(&status, d.status, 4, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  c->state = ST_IDLE;
+  c->win_spin = -1;
+  c->win_rows.clear();
+  if (status != 0) return fail(QMC_ERR_SINGULAR, "a Slater matrix has a zero or non-finite pivot");
+  return QMC_OK;
+}
+
+size_t row_smem(const CrowdDev& d) { return (size_t)(d.ns + 2 * d.kdp + 32) * 8; }
+size_t accept_smem(const CrowdDev& d) { return (size_t)(4 * d.kdp + 16) * 8; }
+
+template <typename T>
+int launch_row_propose_t(qmc_crowd* c, int k, const double* rnew)
+{
+  row_propose_kernel<T><<<c->dev.W, MOVE_NT, row_smem(c->dev), c->stream>>>(c->dev, k, rnew);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+template <typename T>
+int launch_spline_t(qmc_crowd* c)
+{
+  const CrowdDev& d = c->dev;
+  const size_t items = (size_t)d.W * (d.ns / Vec16<T>::W);
+  spline_vgl_kernel<T><<<(unsigned)((items + SPLINE_NT - 1) / SPLINE_NT), SPLINE_NT, 0, c->stream>>>(d);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+template <typename T>
+int launch_ratio_t(qmc_crowd* c, int k, double* ratio, double* grad)
+{
+  ratio_grad_kernel<T><<<c->dev.W, MOVE_NT, 0, c->stream>>>(c->dev, k, ratio, grad);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+template <typename T>
+int launch_rank1_t(qmc_crowd* c, int k)
+{
+  const CrowdDev& d = c->dev;
+  const int rows_per_cta = (RANK1_NT / 32) * RANK1_ROWS_PER_WARP;
+  dim3 grid((d.n + rows_per_cta - 1) / rows_per_cta, d.W);
+  const int nv = (d.ns + 63) / 64;
+  switch (nv) {
+    case 1: rank1_kernel<T, 1><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
+    case 2: rank1_kernel<T, 2><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
+    case 3: rank1_kernel<T, 3><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
+    case 4: rank1_kernel<T, 4><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
+    case 5: case 6: rank1_kernel<T, 6><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
+    case 7: case 8: rank1_kernel<T, 8><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
+    default: rank1_generic_kernel<T><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
+  }
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+template <typename T>
+int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
+{
+  accept_kernel<T><<<c->dev.W, MOVE_NT, accept_smem(c->dev), c->stream>>>(c->dev, k, acc_out);
+  LAUNCH_CHECK(c);
+  if (c->dev.kd == 1) return launch_rank1_t<T>(c, k);
+  return QMC_OK;
+}
+
+int launch_flush(qmc_crowd* c, int spin)
+{
+  const CrowdDev& d = c->dev;
+  const int rows_per_cta = (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP;
+  dim3 grid((d.ns + rows_per_cta - 1) / rows_per_cta, d.W);
+  switch (d.kdp) {
+    case 8: flush_kernel<1><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
+    case 16: flush_kernel<2><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
+    case 32: flush_kernel<4><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
+    case 64: flush_kernel<8><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
+    default: return fail(QMC_ERR_INVALID_ARG, "unsupported padded delay rank %d", d.kdp);
+  }
+  LAUNCH_CHECK(c);
+  CUDA_TRY(cudaMemsetAsync(d.mwin, 0, (size_t)d.W * 4, c->stream));
+  ++c->launches;
+  ++c->flushes;
+  return QMC_OK;
+}
+
+// propose + spline for electron k (qmc_spo_vgl without the optional copies)
+int step_vgl(qmc_crowd* c, int k, const double* rnew)
+{
+  int st = c->is_f64 ? launch_row_propose_t<double>(c, k, rnew) : launch_row_propose_t<float>(c, k, rnew);
+  if (st) return st;
+  return c->is_f64 ? launch_spline_t<double>(c) : launch_spline_t<float>(c);
+}
+int step_ratio(qmc_crowd* c, int k, double* ratio, double* grad)
+{
+  return c->is_f64 ? launch_ratio_t<double>(c, k, ratio, grad) : launch_ratio_t<float>(c, k, ratio, grad);
+}
+int step_accept(qmc_crowd* c, int k, unsigned char* acc)
+{
+  return c->is_f64 ? launch_accept_t<double>(c, k, acc) : launch_accept_t<float>(c, k, acc);
+}
+
+// one full sweep, D:C6 flush schedule; no host synchronisation (capturable)
+int sweep_once(qmc_crowd* c)
+{
+  const CrowdDev& d = c->dev;
+  for (int k = 0; k < d.N; ++k) {
+    int st = step_vgl(c, k, nullptr);
+    if (!st) st = step_ratio(c, k, nullptr, nullptr);
+    if (!st) st = step_accept(c, k, nullptr);
+    if (st) return st;
+    const int kk = k % d.n;
+    if (d.kd > 1 && (((kk + 1) % d.kd) == 0 || kk == d.n - 1)) {
+      st = launch_flush(c, k / d.n);
+      if (st) return st;
+    }
+  }
+  bump_sweep_kernel<<<1, 1, 0, c->stream>>>(d.sweep);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+template <typename TD, typename TS>
+int launch_pack(qmc_crowd* c, TD* dst, const TS* src, size_t nb, int rows, int cols, size_t sb, size_t sr, int scatter)
+{
+  const size_t total = nb * (size_t)rows * cols;
+  if (total == 0) return QMC_OK;
+  size_t blocks = (total + 255) / 256;
+  if (blocks > 148 * 64) blocks = 148 * 64;
+  pack_kernel<TD, TS><<<(unsigned)blocks, 256, 0, c->stream>>>(dst, src, nb, rows, cols, sb, sr, scatter);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+const char* qmc_last_error(void) { return g_err; }
+const char* qmc_version(void) { return "qmc_crowd_b200 0.1 (sm_100a)"; }
+
+size_t qmc_crowd_workspace_bytes(const qmc_crowd_desc* desc)
+{
+  if (check_desc(desc) != QMC_OK) return 0;
+  return carve(desc, nullptr, nullptr);
+}
+
+int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crowd_t** out)
+{
+  if (!out) return fail(QMC_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  int st = check_desc(desc);
+  if (st) return st;
+  if (!pos_dev) return fail(QMC_ERR_INVALID_ARG, "pos_dev is NULL");
+  if (!desc->coefs || ((uintptr_t)desc->coefs & 15)) return fail(QMC_ERR_INVALID_ARG, "coefs must be a 16-byte aligned device pointer");
+  const size_t need = carve(desc, nullptr, nullptr);
+  if (!desc->workspace || ((uintptr_t)desc->workspace & 255) || desc->workspace_bytes < need)
+    return fail(QMC_ERR_WORKSPACE, "workspace must be 256-byte aligned and >= %zu bytes", need);
+  int ndev = 0;
+  CUDA_TRY(cudaGetDeviceCount(&ndev));
+  if (ndev < 1) return fail(QMC_ERR_CUDA, "no CUDA device");
+
+  qmc_crowd* c = new (std::nothrow) qmc_crowd();
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "out of host memory");
+  c->desc = *desc;
+  c->stream = (cudaStream_t)desc->stream;
+  c->is_f64 = desc->coef_dtype;
+  c->elem = desc->coef_dtype ? 8 : 4;
+  c->state = ST_IDLE; c->state_k = -1; c->win_spin = -1;
+  c->proposed = c->flushes = c->launches = 0;
+  c->sweep_host = 0;
+  c->use_graph = 1;
+  c->graph_exec = nullptr;
+  CrowdDev& d = c->dev;
+  memset(&d, 0, sizeof(d));
+  d.W = desc->n_walkers; d.N = desc->n_elec; d.n = d.N / 2; d.M = desc->n_orb;
+  d.ns = (int)align_up((size_t)d.n, 16);
+  d.kd = desc->delay_rank; d.kdp = padded_rank(d.kd);
+  d.walker_id0 = desc->walker_id0;
+  d.seed_lo = (unsigned)(desc->seed & 0xffffffffu); d.seed_hi = (unsigned)(desc->seed >> 32);
+  d.tau = desc->tau; d.sqrt_tau = std::sqrt(desc->tau); d.j2_a = desc->j2_a; d.j2_b = desc->j2_b;
+  const int vw = desc->coef_dtype ? 2 : 4;
+  for (int a = 0; a < 3; ++a) {
+    d.grid[a] = desc->grid[a];
+    d.box[a] = desc->box[a];
+    d.inv_box[a] = 1.0 / desc->box[a];
+    d.inv_h[a] = (double)desc->grid[a] / desc->box[a];
+  }
+  d.orb_stride_v = (unsigned)(desc->orb_stride / vw);
+  d.tab_vecs = d.orb_stride_v;
+  d.coefs = desc->coefs;
+  carve(desc, &d, (char*)desc->workspace);
+
+  auto bail = [&](int code) { delete c; return code; };
+  cudaError_t e = cudaMemsetAsync(desc->workspace, 0, need, c->stream);
+  if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "workspace memset: %s", cudaGetErrorString(e)));
+  e = cudaMemcpyAsync(d.R, pos_dev, (size_t)d.W * d.N * 3 * 8, cudaMemcpyDeviceToDevice, c->stream);
+  if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "position copy: %s", cudaGetErrorString(e)));
+  c->launches += 2;
+  if (row_smem(d) > 48 * 1024) {
+    e = cudaFuncSetAttribute(row_propose_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem(d));
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(row_propose_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem(d));
+    if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
+  }
+  st = rebuild(c);
+  if (st) return bail(st);
+  *out = c;
+  return QMC_OK;
+}
+
+int qmc_crowd_destroy(qmc_crowd_t* c)
+{
+  if (!c) return QMC_OK;
+  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  delete c;
+  return QMC_OK;
+}
+
+int qmc_spo_vgl(qmc_crowd_t* c, int k, const double* rnew_dev, void* phi, void* dphi, void* d2phi)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  const CrowdDev& d = c->dev;
+  if (k < 0 || k >= d.N) return fail(QMC_ERR_INVALID_ARG, "k out of range");
+  const int spin = k / d.n, kk = k % d.n;
+  if (d.kd > 1 && !c->win_rows.empty()) {
+    if (spin != c->win_spin || (int)c->win_rows.size() >= d.kd)
+      return fail(QMC_ERR_STATE, "delayed window is due for qmc_flush_delayed before electron %d", k);
+    for (int r : c->win_rows)
+      if (r == kk) return fail(QMC_ERR_STATE, "electron %d was already proposed in the open delayed window", k);
+  }
+  int st = step_vgl(c, k, rnew_dev);
+  if (st) return st;
+  c->state = ST_HAVE_VGL;
+  c->state_k = k;
+  const size_t ns = (size_t)d.ns;
+  if (c->is_f64) {
+    const double* v = (const double*)d.vgl;
+    if (phi && (st = launch_pack(c, (double*)phi, v, d.W, 1, d.M, 5 * ns, ns, 0))) return st;
+    if (dphi && (st = launch_pack(c, (double*)dphi, v + ns, d.W, 3, d.M, 5 * ns, ns, 0))) return st;
+    if (d2phi && (st = launch_pack(c, (double*)d2phi, v + 4 * ns, d.W, 1, d.M, 5 * ns, ns, 0))) return st;
+  } else {
+    const float* v = (const float*)d.vgl;
+    if (phi && (st = launch_pack(c, (float*)phi, v, d.W, 1, d.M, 5 * ns, ns, 0))) return st;
+    if (dphi && (st = launch_pack(c, (float*)dphi, v + ns, d.W, 3, d.M, 5 * ns, ns, 0))) return st;
+    if (d2phi && (st = launch_pack(c, (float*)d2phi, v + 4 * ns, d.W, 1, d.M, 5 * ns, ns, 0))) return st;
+  }
+  return QMC_OK;
+}
+
+int qmc_ratio_grad(qmc_crowd_t* c, int k, double* ratio, double* grad)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  if (c->state != ST_HAVE_VGL || c->state_k != k)
+    return fail(QMC_ERR_STATE, "qmc_ratio_grad(%d) must follow qmc_spo_vgl(%d)", k, k);
+  int st = step_ratio(c, k, ratio, grad);
+  if (st) return st;
+  c->state = ST_HAVE_RATIO;
+  return QMC_OK;
+}
+
+int qmc_accept_reject(qmc_crowd_t* c, int k, uint8_t* accepted)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  if (c->state != ST_HAVE_RATIO || c->state_k != k)
+    return fail(QMC_ERR_STATE, "qmc_accept_reject(%d) must follow qmc_ratio_grad(%d)", k, k);
+  int st = step_accept(c, k, accepted);
+  if (st) return st;
+  c->state = ST_IDLE;
+  c->proposed += (uint64_t)c->dev.W;
+  if (c->dev.kd > 1) {
+    c->win_spin = k / c->dev.n;
+    c->win_rows.push_back(k % c->dev.n);
+  }
+  return QMC_OK;
+}
+
+int qmc_flush_delayed(qmc_crowd_t* c)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_flush_delayed in the middle of a move");
+  if (c->dev.kd == 1 || c->win_rows.empty()) return QMC_OK;
+  int st = launch_flush(c, c->win_spin);
+  if (st) return st;
+  c->win_rows.clear();
+  c->win_spin = -1;
+  return QMC_OK;
+}
+
+int qmc_sweep(qmc_crowd_t* c, int n_sweeps)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  if (n_sweeps < 0) return fail(QMC_ERR_INVALID_ARG, "n_sweeps < 0");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_sweep in the middle of a move");
+  int st = qmc_flush_delayed(c);
+  if (st) return st;
+  if (c->use_graph && !c->graph_exec && n_sweeps > 0) {
+    // capture one sweep; the sweep index lives in device memory so the graph is replayable
+    cudaStream_t cap = nullptr;
+    CUDA_TRY(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = c->stream;
+    const uint64_t launches0 = c->launches, flushes0 = c->flushes;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+      c->stream = cap;
+      st = sweep_once(c);
+      c->stream = user;
+      e = cudaStreamEndCapture(cap, &graph);
+    }
+    c->launches = launches0;
+    c->flushes = flushes0;
+    if (st == QMC_OK && e == cudaSuccess) e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    cudaStreamDestroy(cap);
+    if (st) return st;
+    if (e != cudaSuccess) { c->graph_exec = nullptr; return fail(QMC_ERR_CUDA, "graph capture: %s", cudaGetErrorString(e)); }
+  }
+  const CrowdDev& d = c->dev;
+  // launches per sweep: 4 (+1 rank-1) per move, 2 per flush, 1 sweep bump
+  const uint64_t flushes_per_sweep = d.kd > 1 ? 2ull * ((d.n + d.kd - 1) / d.kd) : 0;
+  for (int s = 0; s < n_sweeps; ++s) {
+    if (c->use_graph) {
+      CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
+      c->launches += (uint64_t)d.N * (d.kd == 1 ? 5 : 4) + 2 * flushes_per_sweep + 1;
+      c->flushes += flushes_per_sweep;
+    } else {
+      st = sweep_once(c);
+      if (st) return st;
+    }
+    c->proposed += (uint64_t)d.W * d.N;
+    ++c->sweep_host;
+  }
+  return QMC_OK;
+}
+
+int qmc_sweep_host(qmc_crowd_t* c, double* pos_host, int n_sweeps, uint64_t* stats_host)
+{
+  if (!c || !pos_host) return fail(QMC_ERR_INVALID_ARG, "NULL argument");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_sweep_host in the middle of a move");
+  const CrowdDev& d = c->dev;
+  const size_t bytes = (size_t)d.W * d.N * 3 * 8;
+  CUDA_TRY(cudaMemcpyAsync(d.R, pos_host, bytes, cudaMemcpyHostToDevice, c->stream));
+  int st = rebuild(c);
+  if (st) return st;
+  st = qmc_sweep(c, n_sweeps);
+  if (st) return st;
+  CUDA_TRY(cudaMemcpyAsync(pos_host, d.R, bytes, cudaMemcpyDeviceToHost, c->stream));
+  unsigned long long acc = 0;
+  CUDA_TRY(cudaMemcpyAsync(&acc, d.counters, 8, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  if (stats_host) { stats_host[0] = c->proposed; stats_host[1] = acc; stats_host[2] = c->flushes; }
+  return QMC_OK;
+}
+
+int qmc_crowd_get_positions(qmc_crowd_t* c, double* pos_dev)
+{
+  if (!c || !pos_dev) return fail(QMC_ERR_INVALID_ARG, "NULL argument");
+  const CrowdDev& d = c->dev;
+  CUDA_TRY(cudaMemcpyAsync(pos_dev, d.R, (size_t)d.W * d.N * 3 * 8, cudaMemcpyDeviceToDevice, c->stream));
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return QMC_OK;
+}
+
+int qmc_crowd_set_positions(qmc_crowd_t* c, const double* pos_dev)
+{
+  if (!c || !pos_dev) return fail(QMC_ERR_INVALID_ARG, "NULL argument");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "set_positions in the middle of a move");
+  const CrowdDev& d = c->dev;
+  CUDA_TRY(cudaMemcpyAsync(d.R, pos_dev, (size_t)d.W * d.N * 3 * 8, cudaMemcpyDeviceToDevice, c->stream));
+  return rebuild(c);
+}
+
+int qmc_crowd_get_inverse(qmc_crowd_t* c, int spin, double* binv_dev)
+{
+  if (!c || !binv_dev || spin < 0 || spin > 1) return fail(QMC_ERR_INVALID_ARG, "bad argument");
+  const CrowdDev& d = c->dev;
+  const size_t ns = (size_t)d.ns;
+  int st = launch_pack(c, binv_dev, d.Binv + (size_t)spin * ns * ns, d.W, d.n, d.n, 2 * ns * ns, ns, 0);
+  if (st) return st;
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return QMC_OK;
+}
+
+int qmc_crowd_set_inverse(qmc_crowd_t* c, int spin, const double* binv_dev)
+{
+  if (!c || !binv_dev || spin < 0 || spin > 1) return fail(QMC_ERR_INVALID_ARG, "bad argument");
+  if (c->state != ST_IDLE || !c->win_rows.empty()) return fail(QMC_ERR_STATE, "set_inverse needs an empty window");
+  const CrowdDev& d = c->dev;
+  const size_t ns = (size_t)d.ns;
+  int st = launch_pack(c, d.Binv + (size_t)spin * ns * ns, binv_dev, d.W, d.n, d.n, 2 * ns * ns, ns, 1);
+  if (st) return st;
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return QMC_OK;
+}
+
+int qmc_crowd_get_caches(qmc_crowd_t* c, void* dphi_dev, void* d2phi_dev)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  const CrowdDev& d = c->dev;
+  const size_t ns = (size_t)d.ns, nb = (size_t)d.W * d.N;
+  int st = QMC_OK;
+  if (c->is_f64) {
+    const double* s = (const double*)d.cache;
+    if (dphi_dev) st = launch_pack(c, (double*)dphi_dev, s, nb, 3, d.M, 4 * ns, ns, 0);
+    if (!st && d2phi_dev) st = launch_pack(c, (double*)d2phi_dev, s + 3 * ns, nb, 1, d.M, 4 * ns, ns, 0);
+  } else {
+    const float* s = (const float*)d.cache;
+    if (dphi_dev) st = launch_pack(c, (float*)dphi_dev, s, nb, 3, d.M, 4 * ns, ns, 0);
+    if (!st && d2phi_dev) st = launch_pack(c, (float*)d2phi_dev, s + 3 * ns, nb, 1, d.M, 4 * ns, ns, 0);
+  }
+  if (st) return st;
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return QMC_OK;
+}
+
+int qmc_crowd_get_window(qmc_crowd_t* c, int32_t* m_dev, int32_t* rows_dev, double* v_dev, double* c_dev, double* sinv_dev)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  const CrowdDev& d = c->dev;
+  if (d.kd == 1) return fail(QMC_ERR_STATE, "no delayed window with delay_rank 1");
+  const size_t ns = (size_t)d.ns, kdp = (size_t)d.kdp;
+  int st = QMC_OK;
+  if (m_dev) st = launch_pack(c, m_dev, d.mwin, 1, 1, d.W, 0, 0, 0);
+  if (!st && rows_dev) st = launch_pack(c, rows_dev, d.rows, d.W, 1, d.kd, kdp, kdp, 0);
+  if (!st && v_dev) st = launch_pack(c, v_dev, d.V, d.W, d.kd, d.n, kdp * ns, ns, 0);
+  if (!st && c_dev) st = launch_pack(c, c_dev, d.C, d.W, d.kd, d.n, kdp * ns, ns, 0);
+  if (!st && sinv_dev) st = launch_pack(c, sinv_dev, d.Sinv, d.W, d.kd, d.kd, kdp * kdp, kdp, 0);
+  if (st) return st;
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return QMC_OK;
+}
+
+int qmc_crowd_get_move(qmc_crowd_t* c, double* rnew, double* delta, double* g_old, double* g_new, double* rho_d,
+                       double* rho_j, double* p, double* u, double* brow)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  const CrowdDev& d = c->dev;
+  const size_t W = (size_t)d.W;
+  auto cp = [&](double* dst, const double* src, size_t cnt) -> cudaError_t {
+    return dst ? cudaMemcpyAsync(dst, src, cnt * 8, cudaMemcpyDeviceToDevice, c->stream) : cudaSuccess;
+  };
+  CUDA_TRY(cp(rnew, d.rnew, 3 * W));
+  CUDA_TRY(cp(delta, d.delta, 3 * W));
+  CUDA_TRY(cp(g_old, d.g_old, 3 * W));
+  CUDA_TRY(cp(g_new, d.g_new, 3 * W));
+  CUDA_TRY(cp(rho_d, d.rho_d, W));
+  CUDA_TRY(cp(rho_j, d.rho_j, W));
+  CUDA_TRY(cp(p, d.p, W));
+  CUDA_TRY(cp(u, d.u, W));
+  if (brow) {
+    int st = launch_pack(c, brow, d.brow, W, 1, d.n, (size_t)d.ns, (size_t)d.ns, 0);
+    if (st) return st;
+  }
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return QMC_OK;
+}
+
+int qmc_crowd_set_sweep_index(qmc_crowd_t* c, uint32_t s)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  set_u32_kernel<<<1, 1, 0, c->stream>>>(c->dev.sweep, s);
+  LAUNCH_CHECK(c);
+  c->sweep_host = s;
+  return QMC_OK;
+}
+
+int qmc_crowd_stats(qmc_crowd_t* c, uint64_t* proposed, uint64_t* accepted, uint64_t* flushes)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  unsigned long long acc = 0;
+  CUDA_TRY(cudaMemcpyAsync(&acc, c->dev.counters, 8, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  if (proposed) *proposed = c->proposed;
+  if (accepted) *accepted = acc;
+  if (flushes) *flushes = c->flushes;
+  return QMC_OK;
+}
+
+uint64_t qmc_crowd_launch_count(const qmc_crowd_t* c) { return c ? c->launches : 0; }
+
+int qmc_crowd_set_option(qmc_crowd_t* c, int option, int value)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  if (option == QMC_OPT_GRAPH) { c->use_graph = value ? 1 : 0; return QMC_OK; }
+  return fail(QMC_ERR_INVALID_ARG, "unknown option %d", option);
+}
+
+}  // extern "C"
