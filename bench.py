@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- electron moves/s of the crowd move on B200 (BASELINE.json metric).
+
+A "step" is one full sweep of the whole hot path (propose, spline VGL, ratio/grad, accept,
+delayed append, DMMA flush) over one crowd: W x N proposed electron moves (reading A18).
+Workload at N=1: BASELINE.json configs[4] (768 electrons, 80^3 fp32 table, delayed rank 32), the
+largest configuration; it fits one GPU.  Crowd size via --walkers (default 2048).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]        CUDA path, one JSON line
+  python bench.py --impl reference ...                        the oracle on the host cores
+  python bench.py --crowd-sweep                               extra lines: moves/s vs crowd size / rank
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import numpy as np  # noqa: E402
+
+import qmc_inputs as qi  # noqa: E402
+
+METRIC = "electron_moves_per_sec"
+UNIT = "moves/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--cfg", type=int, default=5, help="BASELINE.json config index 1..5")
+    ap.add_argument("--walkers", type=int, default=2048, help="crowd size W per GPU")
+    ap.add_argument("--delay-rank", type=int, default=None)
+    ap.add_argument("--crowd-sweep", action="store_true", help="also print moves/s vs crowd size and delay rank")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ref-walkers", type=int, default=None, help="walkers of the oracle sample (default = cores)")
+    return ap.parse_args()
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return {"hbm_gbs": float(d["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        busy = sorted(sm)[len(sm) // 2:]           # upper half = samples under load
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------------------------
+# the oracle arm: cpu_baseline and --impl reference (the only places bench.py runs oracle/)
+# ----------------------------------------------------------------------------------------------
+def oracle_sample(wl, kd, n_walkers, n_sweeps, coefs=None):
+    """Times oracle_crowd_sweep (as it stands, OpenMP over walkers) on a bounded sample of the
+    workload: the first n_walkers walkers, n_sweeps sweeps.  Returns (moves/s, cores, seconds, accept)."""
+    import oracle
+    coefs = qi.make_coefs(wl) if coefs is None else coefs
+    pos = qi.make_positions(wl, n_walkers)
+    osys = oracle.OracleSystem(wl.n_elec, (wl.grid,) * 3, (wl.box,) * 3, coefs, j2_a=wl.j2_a, j2_b=wl.j2_b,
+                               tau=wl.tau, seed=wl.seed, delay_rank=kd)
+    oc = oracle.OracleCrowd(osys, pos)
+    t0 = time.perf_counter()
+    acc = oc.sweep(n_sweeps)
+    dt = time.perf_counter() - t0
+    moves = n_walkers * wl.n_elec * n_sweeps
+    oc.close()
+    return moves / dt, oracle.num_threads(), dt, acc / moves
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return 0
+    wl = qi.WORKLOADS[args.cfg]
+    kd = args.delay_rank or wl.delay_rank
+    cores = len(os.sched_getaffinity(0))
+    nw = args.ref_walkers or cores
+    coefs = qi.make_coefs(wl)
+    for _ in range(min(args.warmup, 1)):                     # one warm-up sample is enough for a CPU loop
+        oracle_sample(wl, kd, nw, 1, coefs)
+    t_tot, moves, acc = 0.0, 0, 0.0
+    for _ in range(args.steps):
+        v, threads, dt, a = oracle_sample(wl, kd, nw, 1, coefs)
+        t_tot += dt
+        moves += nw * wl.n_elec
+        acc = a
+    value = moves / t_tot
+    sample = f"{nw} walkers x 1 sweep per step of cfg{args.cfg} (N={wl.n_elec}, k={kd}), oracle as it stands"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"cfg{args.cfg}_{wl.n_elec}e_k{kd}", "walkers": nw, "sweeps_per_step": 1},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "accept_fraction": acc, "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------
+# algorithmic work per launch
+# ----------------------------------------------------------------------------------------------
+def algorithmic(wl, W, kd, alpha, el):
+    """Bytes / flops ONE launch of each kernel class moves for a crowd of W walkers, with
+    acceptance fraction alpha (mean window fill at a flush = alpha*kd, mean fill at a move
+    = alpha*(kd-1)/2)."""
+    n = M = wl.n
+    N = wl.n_elec
+    m_move = alpha * (kd - 1) / 2 if kd > 1 else 0.0
+    m_flush = alpha * kd
+    out = {
+        "spline_vgl": {"bytes": W * (64 * M * el + 5 * M * el), "flops": W * 600 * M},
+        "row_propose": {"bytes": W * (8 * n + 2 * 8 * n * m_move + 3 * M * el + 8 * n + 24 * N)},
+        "ratio_grad": {"bytes": W * (8 * n + 4 * M * el + 24 * N)},
+        "accept": {"bytes": alpha * W * (8 * M * el + (8 * n * m_move + 3 * 8 * n + M * el if kd > 1 else 0))},
+        "rank1": {"bytes": alpha * W * 16 * n * n, "flops": alpha * W * 4 * n * n},
+        "flush": {"bytes": W * 16 * n * n, "flops": W * (4 * n * n * m_flush + 2 * n * m_flush ** 2)},
+    }
+    return out
+
+
+# ----------------------------------------------------------------------------------------------
+# the CUDA arm
+# ----------------------------------------------------------------------------------------------
+def make_crowd(wl, W, kd, id0, coefs_dev, dev):
+    import torch
+    import paper_2209_14487_b200 as q
+    pos = qi.make_positions(wl, id0 + W)[id0:]
+    return q.Crowd(coefs_dev, wl.box, torch.from_numpy(np.ascontiguousarray(pos)).to(dev), tau=wl.tau, delay_rank=kd,
+                   j2_a=wl.j2_a, j2_b=wl.j2_b, seed=wl.seed, walker_id0=id0), pos
+
+
+def time_sweeps(crowd, steps, warmup, sync_all):
+    """Device time (CUDA events on the crowd's stream) of `steps` sweeps after `warmup` sweeps."""
+    import torch
+    for _ in range(warmup):
+        crowd.qmc_sweep(1)
+    s0 = crowd.stats()
+    l0 = crowd.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sync_all()
+    e0.record(crowd.stream)
+    for _ in range(steps):
+        crowd.qmc_sweep(1)
+    e1.record(crowd.stream)
+    sync_all()
+    s1 = crowd.stats()
+    return e0.elapsed_time(e1), s1["proposed"] - s0["proposed"], s1["accepted"] - s0["accepted"], crowd.launch_count() - l0
+
+
+def fp64_probe():
+    """cuBLAS DGEMM 8192^3 on this GPU: context for the flush roofline (a probe, not product code)."""
+    import torch
+    a = torch.randn(8192, 8192, dtype=torch.float64, device="cuda")
+    b = torch.randn(8192, 8192, dtype=torch.float64, device="cuda")
+    torch.matmul(a, b)
+    best = 1e9
+    for _ in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); torch.matmul(a, b); e1.record(); torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    return 2 * 8192 ** 3 / (best * 1e-3) / 1e12
+
+
+def run_cuda(args):
+    import torch
+    import paper_2209_14487_b200 as q
+    from paper_2209_14487_b200 import dist as qd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    rank, local_rank, world = qd.env_world()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    qd.init("nccl")
+    wl = qi.WORKLOADS[args.cfg]
+    kd = args.delay_rank or wl.delay_rank
+    W = args.walkers
+    el = 4 if wl.coef_dtype == "f32" else 8
+    id0, _ = qd.walker_slice(rank, world, W)
+    coefs_np = qi.make_coefs(wl)
+    coefs_dev = torch.from_numpy(coefs_np).to(dev)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        qd.barrier()
+        torch.cuda.synchronize()
+
+    t0 = time.perf_counter()
+    crowd, pos = make_crowd(wl, W, kd, id0, coefs_dev, dev)
+    torch.cuda.synchronize()
+    create_s = time.perf_counter() - t0
+
+    with ClockSampler(local_rank) as clk:
+        ms, proposed, accepted, launches = time_sweeps(crowd, args.steps, max(args.warmup, 0), sync_all)
+    ms, (proposed, accepted, launches) = qd.reduce_job(ms, [proposed, accepted, launches], device=dev)
+    value = proposed / (ms * 1e-3)
+    alpha = accepted / max(proposed, 1)
+
+    # per-kernel device time: one more sweep with an event pair around every launch
+    crowd.set_option(q.QMC_OPT_PROFILE, 1)
+    crowd.qmc_sweep(1)
+    prof = crowd.profile()
+    crowd.set_option(q.QMC_OPT_PROFILE, 0)
+    tot_ms = sum(v[0] for v in prof.values()) or 1.0
+    alg = algorithmic(wl, W, kd, alpha, el)
+    pk = peaks()
+    kernels = {}
+    for name, (kms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        avg = kms / cnt
+        ent = {"launches_per_sweep": cnt, "avg_us": 1e3 * avg, "share": kms / tot_ms,
+               "gbs": alg[name]["bytes"] / (avg * 1e-3) / 1e9}
+        ent["hbm_frac"] = ent["gbs"] / pk["hbm_gbs"]
+        if "flops" in alg[name]:
+            ent["tflops"] = alg[name]["flops"] / (avg * 1e-3) / 1e12
+        kernels[name] = ent
+    dom = max(kernels, key=lambda k: kernels[k]["share"])
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "frac": kernels[dom]["gbs"] / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"],
+                "share_of_step": kernels[dom]["share"]}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if kd else "f64", "data": "synthetic",
+        "config": {"workload": f"cfg{args.cfg}_{wl.n_elec}e_k{kd}", "walkers_per_gpu": W, "n_elec": wl.n_elec,
+                   "grid": wl.grid, "table_dtype": wl.coef_dtype, "delay_rank": kd, "sweeps_per_step": 1,
+                   "parallelism": f"walkers sharded over {world} GPU(s), no collective",
+                   "l2": "working set (table + inverses + caches) is far larger than the 126 MB L2; no flush needed"},
+        "accept_fraction": alpha, "gpu_launches": launches, "create_s": create_s,
+        "clocks": clk.summary(), "roofline": roofline, "kernels": kernels,
+    }
+    if rank == 0:
+        try:
+            line["fp64_dgemm_probe_tflops"] = fp64_probe()
+        except Exception as e:  # probe only
+            line["fp64_dgemm_probe_tflops"] = None
+            line["fp64_probe_error"] = str(e)[:80]
+
+    # end to end through the host-buffer call: H2D positions, rebuild, sweep, D2H positions
+    if not args.no_e2e:
+        host = torch.from_numpy(np.ascontiguousarray(pos)).pin_memory()
+        crowd.qmc_sweep_host(host, 1)
+        sync_all()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            crowd.qmc_sweep_host(host, 1)
+        torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) * 1e3
+        e2e_ms, (moves,) = qd.reduce_job(e2e_ms, [W * wl.n_elec * args.steps], device=dev)
+        nbytes = W * wl.n_elec * 24
+        line["e2e"] = {"value": moves / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+                       "d2h_bytes_per_step": nbytes + 8,
+                       "what": "qmc_sweep_host: pinned positions H2D, Slater rebuild + inversion, 1 sweep, positions D2H"}
+    crowd.close()
+    del crowd
+    torch.cuda.empty_cache()
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = len(os.sched_getaffinity(0))
+        nw = args.ref_walkers or cores
+        nw *= 2
+        v, threads, dt, a = oracle_sample(wl, kd, nw, 2, coefs_np)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"{nw} walkers x 2 sweeps of the same workload ({dt:.1f} s wall)",
+                                "accept_fraction": a}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+    if args.crowd_sweep and world == 1:
+        sizes = qi.CFG5_CROWD_SIZES if args.cfg == 5 else (wl.n_walkers // 4, wl.n_walkers // 2, wl.n_walkers)
+        ranks = qi.CFG5_DELAY_RANKS if args.cfg == 5 else (kd,)
+        for k2 in ranks:
+            for W2 in sizes:
+                c2, _ = make_crowd(wl, W2, k2, 0, coefs_dev, dev)
+                ms2, prop2, acc2, _ = time_sweeps(c2, 2, 1, torch.cuda.synchronize)
+                print(json.dumps({"crowd_sweep": True, "walkers": W2, "delay_rank": k2, "value": prop2 / (ms2 * 1e-3),
+                                  "unit": UNIT, "accept_fraction": acc2 / prop2, "ms_per_sweep": ms2 / 2}), flush=True)
+                c2.close()
+                del c2
+                torch.cuda.empty_cache()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -156,6 +156,25 @@ uint64_t qmc_crowd_launch_count(const qmc_crowd_t* crowd);
  * 0 = plain stream launches.                                                                */
 int qmc_crowd_set_option(qmc_crowd_t* crowd, int option, int value);
 #define QMC_OPT_GRAPH 0
+/* option 1 (QMC_OPT_PROFILE): 1 = qmc_sweep and the step calls issue plain launches with a CUDA
+ * event pair around every kernel (measurement aid for bench.py's roofline; adds event overhead,
+ * so throughput numbers are never taken in this mode).                                        */
+#define QMC_OPT_PROFILE 1
+
+/* kernel classes of the hot path, index into qmc_crowd_get_profile's arrays */
+enum {
+  QMC_K_ROW_PROPOSE = 0, /* inverse row with window applied + G_k(R) + proposal (step a0)        */
+  QMC_K_SPLINE_VGL = 1,  /* tricubic B-spline value/gradient/Laplacian (step a1)                 */
+  QMC_K_RATIO_GRAD = 2,  /* determinant + Jastrow ratio and gradient (step a2)                   */
+  QMC_K_ACCEPT = 3,      /* Metropolis decision, cache update, window append (steps a3, a4')     */
+  QMC_K_RANK1 = 4,       /* Sherman-Morrison rank-1 update (step a4)                             */
+  QMC_K_FLUSH = 5,       /* delayed rank-k flush, FP64 DMMA (step a5)                            */
+  QMC_N_KERNEL_CLASSES = 6
+};
+/* Device time (ms, CUDA events on desc.stream) and launch count per kernel class accumulated in
+ * profile mode since the previous call; resets the accumulators.  Synchronous.  ms and count
+ * are HOST arrays of QMC_N_KERNEL_CLASSES entries (either may be NULL).                       */
+int qmc_crowd_get_profile(qmc_crowd_t* crowd, double* ms, uint64_t* count);
 
 const char* qmc_last_error(void); /* thread-local, never NULL */
 const char* qmc_version(void);

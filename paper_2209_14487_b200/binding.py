@@ -15,13 +15,15 @@ _lib = None
 
 QMC_OK, QMC_ERR_INVALID_ARG, QMC_ERR_CUDA, QMC_ERR_WORKSPACE, QMC_ERR_SINGULAR, QMC_ERR_STATE = range(6)
 QMC_OPT_GRAPH = 0
+QMC_OPT_PROFILE = 1
+KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush")
 
 EXPORTS = [
     "qmc_crowd_workspace_bytes", "qmc_crowd_create", "qmc_crowd_destroy", "qmc_spo_vgl", "qmc_ratio_grad",
     "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_crowd_get_positions",
     "qmc_crowd_set_positions", "qmc_crowd_get_inverse", "qmc_crowd_set_inverse", "qmc_crowd_get_caches",
     "qmc_crowd_get_window", "qmc_crowd_get_move", "qmc_crowd_set_sweep_index", "qmc_crowd_stats",
-    "qmc_crowd_launch_count", "qmc_crowd_set_option", "qmc_last_error", "qmc_version",
+    "qmc_crowd_launch_count", "qmc_crowd_set_option", "qmc_crowd_get_profile", "qmc_last_error", "qmc_version",
 ]
 
 
@@ -81,6 +83,7 @@ def load():
     L.qmc_crowd_launch_count.argtypes = [vp]
     L.qmc_crowd_launch_count.restype = C.c_uint64
     L.qmc_crowd_set_option.argtypes = [vp, ip, ip]
+    L.qmc_crowd_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
     L.qmc_last_error.restype = C.c_char_p
     L.qmc_version.restype = C.c_char_p
     _lib = L
@@ -242,6 +245,12 @@ class Crowd:
 
     def launch_count(self):
         return int(load().qmc_crowd_launch_count(self._h))
+
+    def profile(self):
+        """{kernel class: (total ms, launches)} recorded in QMC_OPT_PROFILE mode since the last call."""
+        ms, cnt = (C.c_double * len(KERNEL_CLASSES))(), (C.c_uint64 * len(KERNEL_CLASSES))()
+        _check(load().qmc_crowd_get_profile(self._h, ms, cnt))
+        return {name: (ms[i], int(cnt[i])) for i, name in enumerate(KERNEL_CLASSES)}
 
     def set_option(self, option, value):
         _check(load().qmc_crowd_set_option(self._h, option, value))

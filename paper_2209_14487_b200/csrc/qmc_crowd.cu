@@ -47,6 +47,8 @@ int fail(int code, const char* fmt, ...)
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+struct ProfScope;
+
 enum StepState { ST_IDLE = 0, ST_HAVE_VGL = 1, ST_HAVE_RATIO = 2 };
 
 }  // namespace
@@ -64,10 +66,41 @@ struct qmc_crowd {
   uint32_t sweep_host;
   int use_graph;
   cudaGraphExec_t graph_exec;
-  unsigned char* acc_scratch;  // unused output sink
+  // QMC_OPT_PROFILE: CUDA-event pairs around every kernel of the plain-launch sweep
+  int profile;
+  std::vector<cudaEvent_t> ev;      // pool, pairs (begin, end)
+  std::vector<int> ev_class;        // kernel class of pair i
+  size_t ev_used;                   // pairs recorded since the last qmc_crowd_get_profile
+  double prof_ms[QMC_N_KERNEL_CLASSES];
+  uint64_t prof_cnt[QMC_N_KERNEL_CLASSES];
 };
 
 namespace {
+
+// Records an event pair around the launches issued while it is alive (profile mode only).
+struct ProfScope {
+  qmc_crowd* c;
+  size_t idx;
+  bool on;
+  ProfScope(qmc_crowd* c_, int cls) : c(c_), idx(0), on(c_->profile != 0)
+  {
+    if (!on) return;
+    if (c->ev_used * 2 + 2 > c->ev.size()) {
+      cudaEvent_t a = nullptr, b = nullptr;
+      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { on = false; return; }
+      c->ev.push_back(a);
+      c->ev.push_back(b);
+      c->ev_class.push_back(cls);
+    }
+    idx = c->ev_used++;
+    c->ev_class[idx] = cls;
+    cudaEventRecord(c->ev[2 * idx], c->stream);
+  }
+  ~ProfScope()
+  {
+    if (on) cudaEventRecord(c->ev[2 * idx + 1], c->stream);
+  }
+};
 
 int padded_rank(int kd)
 {
@@ -245,9 +278,15 @@ int launch_rank1_t(qmc_crowd* c, int k)
 template <typename T>
 int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
 {
-  accept_kernel<T><<<c->dev.W, MOVE_NT, accept_smem(c->dev), c->stream>>>(c->dev, k, acc_out);
-  LAUNCH_CHECK(c);
-  if (c->dev.kd == 1) return launch_rank1_t<T>(c, k);
+  {
+    ProfScope ps(c, QMC_K_ACCEPT);
+    accept_kernel<T><<<c->dev.W, MOVE_NT, accept_smem(c->dev), c->stream>>>(c->dev, k, acc_out);
+    LAUNCH_CHECK(c);
+  }
+  if (c->dev.kd == 1) {
+    ProfScope ps(c, QMC_K_RANK1);
+    return launch_rank1_t<T>(c, k);
+  }
   return QMC_OK;
 }
 
@@ -256,6 +295,7 @@ int launch_flush(qmc_crowd* c, int spin)
   const CrowdDev& d = c->dev;
   const int rows_per_cta = (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP;
   dim3 grid((d.ns + rows_per_cta - 1) / rows_per_cta, d.W);
+  ProfScope ps(c, QMC_K_FLUSH);
   switch (d.kdp) {
     case 8: flush_kernel<1><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
     case 16: flush_kernel<2><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
@@ -273,12 +313,18 @@ int launch_flush(qmc_crowd* c, int spin)
 // propose + spline for electron k (qmc_spo_vgl without the optional copies)
 int step_vgl(qmc_crowd* c, int k, const double* rnew)
 {
-  int st = c->is_f64 ? launch_row_propose_t<double>(c, k, rnew) : launch_row_propose_t<float>(c, k, rnew);
+  int st;
+  {
+    ProfScope ps(c, QMC_K_ROW_PROPOSE);
+    st = c->is_f64 ? launch_row_propose_t<double>(c, k, rnew) : launch_row_propose_t<float>(c, k, rnew);
+  }
   if (st) return st;
+  ProfScope ps(c, QMC_K_SPLINE_VGL);
   return c->is_f64 ? launch_spline_t<double>(c) : launch_spline_t<float>(c);
 }
 int step_ratio(qmc_crowd* c, int k, double* ratio, double* grad)
 {
+  ProfScope ps(c, QMC_K_RATIO_GRAD);
   return c->is_f64 ? launch_ratio_t<double>(c, k, ratio, grad) : launch_ratio_t<float>(c, k, ratio, grad);
 }
 int step_accept(qmc_crowd* c, int k, unsigned char* acc)
@@ -360,6 +406,9 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   c->sweep_host = 0;
   c->use_graph = 1;
   c->graph_exec = nullptr;
+  c->profile = 0;
+  c->ev_used = 0;
+  for (int i = 0; i < QMC_N_KERNEL_CLASSES; ++i) { c->prof_ms[i] = 0.0; c->prof_cnt[i] = 0; }
   CrowdDev& d = c->dev;
   memset(&d, 0, sizeof(d));
   d.W = desc->n_walkers; d.N = desc->n_elec; d.n = d.N / 2; d.M = desc->n_orb;
@@ -402,6 +451,7 @@ int qmc_crowd_destroy(qmc_crowd_t* c)
 {
   if (!c) return QMC_OK;
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   delete c;
   return QMC_OK;
 }
@@ -483,7 +533,7 @@ int qmc_sweep(qmc_crowd_t* c, int n_sweeps)
   if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_sweep in the middle of a move");
   int st = qmc_flush_delayed(c);
   if (st) return st;
-  if (c->use_graph && !c->graph_exec && n_sweeps > 0) {
+  if (c->use_graph && !c->profile && !c->graph_exec && n_sweeps > 0) {
     // capture one sweep; the sweep index lives in device memory so the graph is replayable
     cudaStream_t cap = nullptr;
     CUDA_TRY(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
@@ -509,7 +559,7 @@ int qmc_sweep(qmc_crowd_t* c, int n_sweeps)
   // launches per sweep: 4 (+1 rank-1) per move, 2 per flush, 1 sweep bump
   const uint64_t flushes_per_sweep = d.kd > 1 ? 2ull * ((d.n + d.kd - 1) / d.kd) : 0;
   for (int s = 0; s < n_sweeps; ++s) {
-    if (c->use_graph) {
+    if (c->use_graph && !c->profile) {
       CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
       c->launches += (uint64_t)d.N * (d.kd == 1 ? 5 : 4) + 2 * flushes_per_sweep + 1;
       c->flushes += flushes_per_sweep;
@@ -666,12 +716,33 @@ int qmc_crowd_stats(qmc_crowd_t* c, uint64_t* proposed, uint64_t* accepted, uint
   return QMC_OK;
 }
 
+int qmc_crowd_get_profile(qmc_crowd_t* c, double* ms, uint64_t* count)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  for (size_t i = 0; i < c->ev_used; ++i) {
+    float t = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&t, c->ev[2 * i], c->ev[2 * i + 1]));
+    c->prof_ms[c->ev_class[i]] += (double)t;
+    c->prof_cnt[c->ev_class[i]] += 1;
+  }
+  c->ev_used = 0;
+  for (int i = 0; i < QMC_N_KERNEL_CLASSES; ++i) {
+    if (ms) ms[i] = c->prof_ms[i];
+    if (count) count[i] = c->prof_cnt[i];
+    c->prof_ms[i] = 0.0;
+    c->prof_cnt[i] = 0;
+  }
+  return QMC_OK;
+}
+
 uint64_t qmc_crowd_launch_count(const qmc_crowd_t* c) { return c ? c->launches : 0; }
 
 int qmc_crowd_set_option(qmc_crowd_t* c, int option, int value)
 {
   if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
   if (option == QMC_OPT_GRAPH) { c->use_graph = value ? 1 : 0; return QMC_OK; }
+  if (option == QMC_OPT_PROFILE) { c->profile = value ? 1 : 0; return QMC_OK; }
   return fail(QMC_ERR_INVALID_ARG, "unknown option %d", option);
 }
 
