@@ -117,7 +117,7 @@ __device__ __forceinline__ double u01(unsigned x) { return ((double)x + 0.5) * (
 // B[l%4][l/4] and D[l/4][2(l%4) + {0,1}].  SASS: DMMA.8x8x4.
 __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b)
 {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c[0]), "+d"(c[1])
                : "d"(a), "d"(b));
 }

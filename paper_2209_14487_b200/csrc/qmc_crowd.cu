@@ -65,6 +65,7 @@ struct qmc_crowd {
   uint64_t proposed, flushes, launches;
   uint32_t sweep_host;
   int use_graph;
+  int flush_attr_set;
   cudaGraphExec_t graph_exec;
   // QMC_OPT_PROFILE: CUDA-event pairs around every kernel of the plain-launch sweep
   int profile;
@@ -296,13 +297,37 @@ int launch_flush(qmc_crowd* c, int spin)
   const int rows_per_cta = (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP;
   dim3 grid((d.ns + rows_per_cta - 1) / rows_per_cta, d.W);
   ProfScope ps(c, QMC_K_FLUSH);
+  const int fcols = FINALIZE_NT / (d.kdp > 32 ? d.kdp / 32 : 1);
+  dim3 fgrid((d.ns + fcols - 1) / fcols, d.W);
+  const size_t fsm = (size_t)d.kdp * d.kdp * 8;
+  const size_t flush_smem = (size_t)FLUSH_DEPTH * (FLUSH_WARPS * FLUSH_STRIP_BYTES + (size_t)d.kdp * 128);
+  if (flush_smem > 48 * 1024 && !c->flush_attr_set) {
+    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
+    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
+    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
+    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
+    c->flush_attr_set = 1;
+  }
   switch (d.kdp) {
-    case 8: flush_kernel<1><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
-    case 16: flush_kernel<2><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
-    case 32: flush_kernel<4><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
-    case 64: flush_kernel<8><<<grid, FLUSH_NT, 0, c->stream>>>(d, spin); break;
+    case 8:
+      flush_finalize_kernel<8><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_kernel<1><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
+      break;
+    case 16:
+      flush_finalize_kernel<16><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_kernel<2><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
+      break;
+    case 32:
+      flush_finalize_kernel<32><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_kernel<4><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
+      break;
+    case 64:
+      flush_finalize_kernel<64><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_kernel<8><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
+      break;
     default: return fail(QMC_ERR_INVALID_ARG, "unsupported padded delay rank %d", d.kdp);
   }
+  ++c->launches;
   LAUNCH_CHECK(c);
   CUDA_TRY(cudaMemsetAsync(d.mwin, 0, (size_t)d.W * 4, c->stream));
   ++c->launches;
@@ -405,6 +430,7 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   c->proposed = c->flushes = c->launches = 0;
   c->sweep_host = 0;
   c->use_graph = 1;
+  c->flush_attr_set = 0;
   c->graph_exec = nullptr;
   c->profile = 0;
   c->ev_used = 0;
@@ -556,12 +582,12 @@ int qmc_sweep(qmc_crowd_t* c, int n_sweeps)
     if (e != cudaSuccess) { c->graph_exec = nullptr; return fail(QMC_ERR_CUDA, "graph capture: %s", cudaGetErrorString(e)); }
   }
   const CrowdDev& d = c->dev;
-  // launches per sweep: 4 (+1 rank-1) per move, 2 per flush, 1 sweep bump
+  // launches per sweep: 4 (+1 rank-1) per move, 3 per flush, 1 sweep bump
   const uint64_t flushes_per_sweep = d.kd > 1 ? 2ull * ((d.n + d.kd - 1) / d.kd) : 0;
   for (int s = 0; s < n_sweeps; ++s) {
     if (c->use_graph && !c->profile) {
       CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
-      c->launches += (uint64_t)d.N * (d.kd == 1 ? 5 : 4) + 2 * flushes_per_sweep + 1;
+      c->launches += (uint64_t)d.N * (d.kd == 1 ? 5 : 4) + 3 * flushes_per_sweep + 1;
       c->flushes += flushes_per_sweep;
     } else {
       st = sweep_once(c);
