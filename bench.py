@@ -166,11 +166,17 @@ def algorithmic(wl, W, kd, alpha, el):
     N = wl.n_elec
     m_move = alpha * (kd - 1) / 2 if kd > 1 else 0.0
     m_flush = alpha * kd
+    ratio_b = W * (8 * n + 4 * M * el + 24 * N)
+    accept_b = alpha * W * (8 * M * el + (8 * n * m_move + 3 * 8 * n + M * el if kd > 1 else 0))
+    row_b = W * (8 * n + 2 * 8 * n * m_move + 3 * M * el + 8 * n + 24 * N)
     out = {
         "spline_vgl": {"bytes": W * (64 * M * el + 5 * M * el), "flops": W * 600 * M},
-        "row_propose": {"bytes": W * (8 * n + 2 * 8 * n * m_move + 3 * M * el + 8 * n + 24 * N)},
-        "ratio_grad": {"bytes": W * (8 * n + 4 * M * el + 24 * N)},
-        "accept": {"bytes": alpha * W * (8 * M * el + (8 * n * m_move + 3 * 8 * n + M * el if kd > 1 else 0))},
+        "row_propose": {"bytes": row_b},
+        "ratio_grad": {"bytes": ratio_b},
+        "accept": {"bytes": accept_b},
+        "ratio_accept": {"bytes": ratio_b + accept_b},
+        # fused ratio(k) + accept(k) + row(k+1): C rows and positions are needed once, not twice
+        "fused_move": {"bytes": ratio_b + accept_b + row_b - alpha * W * 8 * n * m_move - W * 24 * N},
         "rank1": {"bytes": alpha * W * 16 * n * n, "flops": alpha * W * 4 * n * n},
         "flush": {"bytes": W * 16 * n * n, "flops": W * (4 * n * n * m_flush + 2 * n * m_flush ** 2)},
     }

@@ -169,7 +169,9 @@ enum {
   QMC_K_ACCEPT = 3,      /* Metropolis decision, cache update, window append (steps a3, a4')     */
   QMC_K_RANK1 = 4,       /* Sherman-Morrison rank-1 update (step a4)                             */
   QMC_K_FLUSH = 5,       /* delayed rank-k flush, FP64 DMMA (step a5)                            */
-  QMC_N_KERNEL_CLASSES = 6
+  QMC_K_RATIO_ACCEPT = 6,/* qmc_sweep only: ratio_grad + accept of electron k in one kernel      */
+  QMC_K_FUSED_MOVE = 7,  /* qmc_sweep only: ratio_grad + accept of k, row/proposal of k+1        */
+  QMC_N_KERNEL_CLASSES = 8
 };
 /* Device time (ms, CUDA events on desc.stream) and launch count per kernel class accumulated in
  * profile mode since the previous call; resets the accumulators.  Synchronous.  ms and count

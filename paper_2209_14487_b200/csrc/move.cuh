@@ -7,7 +7,17 @@
 
 namespace qmc {
 
-constexpr int MOVE_NT = 128;
+#ifndef QMC_MOVE_NT
+#define QMC_MOVE_NT 128
+#endif
+#ifndef QMC_MOVE_DOT_ROWS
+#define QMC_MOVE_DOT_ROWS 2
+#endif
+#ifndef QMC_MOVE_PREFETCH
+#define QMC_MOVE_PREFETCH 0
+#endif
+constexpr int MOVE_NT = QMC_MOVE_NT;
+constexpr int MOVE_RED = 8 * (MOVE_NT / 32) < 32 ? 32 : 8 * (MOVE_NT / 32);  // doubles of reduction scratch
 
 // D:C3: one pair term of the two-body Jastrow for electron k placed at rk against electron i.
 // u(r) = a r/(1 + b r), u'(r) = a/(1 + b r)^2, minimum image d_c <- d_c - L rint(d_c/L).
@@ -33,21 +43,50 @@ __device__ __forceinline__ void j2_pair(const CrowdDev& d, const double (&rk)[3]
   }
 }
 
+// out[l] = mat[l,:] . x for l in [0, nrows), mat row-major with stride ns (ns % 2 == 0), x in shared
+// memory.  A warp takes MOVE_DOT_ROWS rows at a time and keeps their loads in flight together
+// (one DRAM round trip per group instead of one per row); then shuffle-reduces each row.
+constexpr int MOVE_DOT_ROWS = QMC_MOVE_DOT_ROWS;
+template <typename F>
+__device__ __forceinline__ void rows_dot(const double* __restrict__ mat, int ns, int nrows, const double* x_s, F&& store)
+{
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int l0 = warp * MOVE_DOT_ROWS; l0 < nrows; l0 += (MOVE_NT / 32) * MOVE_DOT_ROWS) {
+    double acc[MOVE_DOT_ROWS];
+#pragma unroll
+    for (int r = 0; r < MOVE_DOT_ROWS; ++r) acc[r] = 0.0;
+#pragma unroll 2
+    for (int jj = lane; jj < ns / 2; jj += 32) {
+      const double x0 = x_s[2 * jj], x1 = x_s[2 * jj + 1];
+      double2 v[MOVE_DOT_ROWS];
+#pragma unroll
+      for (int r = 0; r < MOVE_DOT_ROWS; ++r)
+        v[r] = (l0 + r < nrows) ? reinterpret_cast<const double2*>(mat + (size_t)(l0 + r) * ns)[jj] : make_double2(0.0, 0.0);
+#pragma unroll
+      for (int r = 0; r < MOVE_DOT_ROWS; ++r) acc[r] = fma(v[r].x, x0, fma(v[r].y, x1, acc[r]));
+    }
+#pragma unroll
+    for (int r = 0; r < MOVE_DOT_ROWS; ++r) {
+      const double t = warp_sum(acc[r]);
+      if (lane == 0 && l0 + r < nrows) store(l0 + r, t);
+    }
+  }
+}
+
 // ---- qmc_spo_vgl steps (a)+(b) -----------------------------------------------------------
 // (a) b = B0[k,:] - C^T (Sinv p), p_l = V[l,:].B0[k,:] - [rows[l]==k]   (D:C6)
 //     G_k(R) = b . grad phi(r_k) [cache] + grad_k ln Psi_J(R)             (D:C2, C3, A13)
 // (b) Delta = fl32(tau G + sqrt(tau) chi), r' = r_k + Delta               (D:C4, C7)
-// dynamic smem: (ns + 2 kdp + 32) doubles
+// sm: (ns + 2 kdp + MOVE_RED) doubles
 template <typename T>
-__global__ void __launch_bounds__(MOVE_NT) row_propose_kernel(CrowdDev d, int k, const double* __restrict__ rnew_given)
+__device__ __forceinline__ void dev_row_propose(const CrowdDev& d, int w, int k, const double* __restrict__ rnew_given,
+                                                double* sm)
 {
-  extern __shared__ double sm[];
   const int ns = d.ns, kdp = d.kdp, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   double* b_s = sm;
   double* p_s = b_s + ns;
   double* y_s = p_s + kdp;
   double* red = y_s + kdp;
-  const int w = blockIdx.x;
   const int spin = k / d.n, kk = k - spin * d.n;
   const double* B0 = d.Binv + ((size_t)w * 2 + spin) * ns * ns;
   const int m = d.kd > 1 ? d.mwin[w] : 0;
@@ -59,24 +98,16 @@ __global__ void __launch_bounds__(MOVE_NT) row_propose_kernel(CrowdDev d, int k,
     const double* C = d.C + (size_t)w * kdp * ns;
     const double* Sinv = d.Sinv + (size_t)w * kdp * kdp;
     const int* rows = d.rows + (size_t)w * kdp;
-    for (int l = warp; l < m; l += MOVE_NT / 32) {
-      const double2* v2 = reinterpret_cast<const double2*>(V + (size_t)l * ns);
-      double acc = 0.0;
-      for (int jj = lane; jj < ns / 2; jj += 32) {
-        const double2 v = v2[jj];
-        acc = fma(v.x, b_s[2 * jj], acc);
-        acc = fma(v.y, b_s[2 * jj + 1], acc);
-      }
-      acc = warp_sum(acc);
-      if (lane == 0) {
-        const double pl = acc - (rows[l] == kk ? 1.0 : 0.0);
-        p_s[l] = pl;
-        d.pvec[(size_t)w * kdp + l] = pl;
-      }
-    }
+    double* pvec = d.pvec + (size_t)w * kdp;
+    rows_dot(V, ns, m, b_s, [&](int l, double acc) {
+      const double pl = acc - (rows[l] == kk ? 1.0 : 0.0);
+      p_s[l] = pl;
+      pvec[l] = pl;
+    });
     __syncthreads();
     for (int l = tid; l < m; l += MOVE_NT) {
       double y = 0.0;
+#pragma unroll 8
       for (int q = 0; q < m; ++q) y = fma(Sinv[(size_t)l * kdp + q], p_s[q], y);
       y_s[l] = y;
       d.yvec[(size_t)w * kdp + l] = y;
@@ -84,7 +115,7 @@ __global__ void __launch_bounds__(MOVE_NT) row_propose_kernel(CrowdDev d, int k,
     __syncthreads();
     for (int jj = tid; jj < ns / 2; jj += MOVE_NT) {
       double2 acc = make_double2(b_s[2 * jj], b_s[2 * jj + 1]);
-#pragma unroll 4
+#pragma unroll 8
       for (int l = 0; l < m; ++l) {
         const double2 c = reinterpret_cast<const double2*>(C + (size_t)l * ns)[jj];
         acc.x = fma(-y_s[l], c.x, acc.x);
@@ -148,12 +179,12 @@ __global__ void __launch_bounds__(MOVE_NT) row_propose_kernel(CrowdDev d, int k,
 
 // ---- qmc_ratio_grad ------------------------------------------------------------------------
 // rho_D = b . phi(r'); grad = (b . grad phi(r'))/rho_D + grad_k ln Psi_J(R'); rho_J (D:C2, C3)
+// sm: MOVE_RED doubles
 template <typename T>
-__global__ void __launch_bounds__(MOVE_NT) ratio_grad_kernel(CrowdDev d, int k, double* __restrict__ ratio_out,
-                                                             double* __restrict__ grad_out)
+__device__ __forceinline__ void dev_ratio_grad(const CrowdDev& d, int w, int k, double* __restrict__ ratio_out,
+                                               double* __restrict__ grad_out, double* red)
 {
-  __shared__ double red[8 * MOVE_NT / 32];
-  const int ns = d.ns, tid = threadIdx.x, w = blockIdx.x;
+  const int ns = d.ns, tid = threadIdx.x;
   const double* b = d.brow + (size_t)w * ns;
   const T* vgl = static_cast<const T*>(d.vgl) + (size_t)w * 5 * ns;
   double v[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
@@ -193,13 +224,13 @@ __global__ void __launch_bounds__(MOVE_NT) ratio_grad_kernel(CrowdDev d, int k, 
 // (D:C4); accept <=> u < p.  On accept with a delayed window (D:C6): V[m] = phi', C[m] = B0[k,:],
 // S^-1 bordered with column p (kept by row_propose), row q_l = C[l,:].phi' and Schur complement
 // sigma = B0[k,:].phi' - q.(Sinv p) (= rho_D up to rounding).
-// dynamic smem: (4 kdp + 16) doubles
+// sm: (ns + 3 kdp + 16) doubles
 template <typename T>
-__global__ void __launch_bounds__(MOVE_NT) accept_kernel(CrowdDev d, int k, unsigned char* __restrict__ acc_out)
+__device__ __forceinline__ void dev_accept(const CrowdDev& d, int w, int k, unsigned char* __restrict__ acc_out,
+                                           double* sm)
 {
-  extern __shared__ double sm[];
   __shared__ int s_acc;
-  const int ns = d.ns, kdp = d.kdp, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, w = blockIdx.x;
+  const int ns = d.ns, kdp = d.kdp, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid == 0) {
     const double tau = d.tau;
     double f2 = 0.0, b2 = 0.0;
@@ -245,22 +276,21 @@ __global__ void __launch_bounds__(MOVE_NT) accept_kernel(CrowdDev d, int k, unsi
   double* z_s = q_s + kdp;     // [kdp]  z = q^T Sinv
   double* y_s = z_s + kdp;     // [kdp]  y = Sinv p
   double* misc = y_s + kdp;    // corner, sigma
+  double* phi_s = misc + 16;   // [ns]   phi' widened to fp64 (padding columns are zero)
   for (int j = tid; j < ns; j += MOVE_NT) {
-    V[(size_t)m * ns + j] = (double)vgl[j];
+    const double ph = (double)vgl[j];
+    phi_s[j] = ph;
+    V[(size_t)m * ns + j] = ph;
     C[(size_t)m * ns + j] = B0k[j];
   }
-  // q_l for l < m, and the corner B0[k,:].phi' as "row m"
-  for (int l = warp; l <= m; l += MOVE_NT / 32) {
-    const double* row = (l < m) ? C + (size_t)l * ns : B0k;
-    double acc = 0.0;
-    for (int j = lane; j < d.M; j += 32) acc = fma(row[j], (double)vgl[j], acc);
-    acc = warp_sum(acc);
-    if (lane == 0) { if (l < m) q_s[l] = acc; else misc[0] = acc; }
-  }
+  __syncthreads();
+  // q_l = C[l,:].phi' for l < m, and the corner B0[k,:].phi' (= row m of C, just written)
+  rows_dot(C, ns, m + 1, phi_s, [&](int l, double acc) { if (l < m) q_s[l] = acc; else misc[0] = acc; });
   for (int l = tid; l < m; l += MOVE_NT) y_s[l] = d.yvec[(size_t)w * kdp + l];
   __syncthreads();
   for (int l = tid; l < m; l += MOVE_NT) {
     double z = 0.0;
+#pragma unroll 8
     for (int q = 0; q < m; ++q) z = fma(q_s[q], Sinv[(size_t)q * kdp + l], z);
     z_s[l] = z;
   }
@@ -283,6 +313,68 @@ __global__ void __launch_bounds__(MOVE_NT) accept_kernel(CrowdDev d, int k, unsi
     Sinv[(size_t)m * kdp + m] = inv_sigma;
     d.rows[(size_t)w * kdp + m] = kk;
     d.mwin[w] = m + 1;
+  }
+}
+
+// ---- kernels: the three step calls, and their fusions used by qmc_sweep ------------------------
+// Walkers never interact, so nothing forces a kernel boundary between accept(k) and the row/proposal
+// of electron k+1 of the same walker: move_fused_kernel does ratio(k), accept(k), row_propose(k+1) in
+// one CTA, so the window rows C (read for the append and again for the next row), V and the positions
+// come from DRAM once.  The device functions are the ones the step kernels run.
+// dynamic smem of all of them: move_smem_doubles(d) doubles
+template <typename T>
+__global__ void __launch_bounds__(MOVE_NT) row_propose_kernel(CrowdDev d, int k, const double* __restrict__ rnew_given)
+{
+  extern __shared__ double sm[];
+  dev_row_propose<T>(d, blockIdx.x, k, rnew_given, sm);
+}
+template <typename T>
+__global__ void __launch_bounds__(MOVE_NT) ratio_grad_kernel(CrowdDev d, int k, double* __restrict__ ratio_out,
+                                                             double* __restrict__ grad_out)
+{
+  extern __shared__ double sm[];
+  dev_ratio_grad<T>(d, blockIdx.x, k, ratio_out, grad_out, sm);
+}
+template <typename T>
+__global__ void __launch_bounds__(MOVE_NT) accept_kernel(CrowdDev d, int k, unsigned char* __restrict__ acc_out)
+{
+  extern __shared__ double sm[];
+  dev_accept<T>(d, blockIdx.x, k, acc_out, sm);
+}
+// ratio(k) + accept(k); with NEXT also row_propose(k + 1) (same spin block, no flush in between)
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// mmax = upper bound of the window fill after this move (proposals of the open window incl. k)
+template <typename T, bool NEXT>
+__global__ void __launch_bounds__(MOVE_NT) move_fused_kernel(CrowdDev d, int k, int mmax)
+{
+  extern __shared__ double sm[];
+  const int w = blockIdx.x;
+  if (NEXT && QMC_MOVE_PREFETCH) {
+    // The CTA is a chain of short dependent phases, each a DRAM round trip.  Everything the later
+    // phases will read is known now: pull it into L2 while the ratio phase runs (no registers held).
+    const int ns = d.ns, lpr = ns / 16;              // 128-byte lines per fp64 row
+    const int spin = k / d.n, kk = k - spin * d.n;
+    const char* V = reinterpret_cast<const char*>(d.V + (size_t)w * d.kdp * ns);
+    const char* C = reinterpret_cast<const char*>(d.C + (size_t)w * d.kdp * ns);
+    const int nl = mmax * lpr;
+    for (int e = threadIdx.x; e < nl; e += MOVE_NT) {
+      prefetch_l2(V + (size_t)e * 128);
+      prefetch_l2(C + (size_t)e * 128);
+    }
+    const char* b0 = reinterpret_cast<const char*>(d.Binv + (((size_t)w * 2 + spin) * ns + kk) * ns);
+    const char* cache = static_cast<const char*>(d.cache) + ((size_t)w * d.N + k + 1) * 4 * ns * sizeof(T);
+    for (int e = threadIdx.x; e < 2 * lpr; e += MOVE_NT) prefetch_l2(b0 + (size_t)e * 128);   // rows kk and kk+1
+    for (int e = threadIdx.x; e < (int)(3 * ns * sizeof(T) / 128); e += MOVE_NT) prefetch_l2(cache + (size_t)e * 128);
+    const char* sinv = reinterpret_cast<const char*>(d.Sinv + (size_t)w * d.kdp * d.kdp);
+    for (int e = threadIdx.x; e < mmax * d.kdp / 16; e += MOVE_NT) prefetch_l2(sinv + (size_t)e * 128);
+  }
+  dev_ratio_grad<T>(d, w, k, nullptr, nullptr, sm);
+  __syncthreads();
+  dev_accept<T>(d, w, k, nullptr, sm);
+  if (NEXT) {
+    __syncthreads();
+    dev_row_propose<T>(d, w, k + 1, nullptr, sm);
   }
 }
 

@@ -65,7 +65,7 @@ struct qmc_crowd {
   uint64_t proposed, flushes, launches;
   uint32_t sweep_host;
   int use_graph;
-  int flush_attr_set;
+  uint64_t graph_launches, graph_flushes;  // per replay of the captured sweep
   cudaGraphExec_t graph_exec;
   // QMC_OPT_PROFILE: CUDA-event pairs around every kernel of the plain-launch sweep
   int profile;
@@ -227,13 +227,17 @@ int rebuild(qmc_crowd* c)
   return QMC_OK;
 }
 
-size_t row_smem(const CrowdDev& d) { return (size_t)(d.ns + 2 * d.kdp + 32) * 8; }
-size_t accept_smem(const CrowdDev& d) { return (size_t)(4 * d.kdp + 16) * 8; }
+// dynamic smem of every move kernel: the largest need of the three device functions
+size_t move_smem(const CrowdDev& d)
+{
+  const size_t row = (size_t)d.ns + 2 * d.kdp + MOVE_RED, acc = (size_t)d.ns + 3 * d.kdp + 16;
+  return (row > acc ? row : acc) * 8;
+}
 
 template <typename T>
 int launch_row_propose_t(qmc_crowd* c, int k, const double* rnew)
 {
-  row_propose_kernel<T><<<c->dev.W, MOVE_NT, row_smem(c->dev), c->stream>>>(c->dev, k, rnew);
+  row_propose_kernel<T><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k, rnew);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
@@ -251,7 +255,7 @@ int launch_spline_t(qmc_crowd* c)
 template <typename T>
 int launch_ratio_t(qmc_crowd* c, int k, double* ratio, double* grad)
 {
-  ratio_grad_kernel<T><<<c->dev.W, MOVE_NT, 0, c->stream>>>(c->dev, k, ratio, grad);
+  ratio_grad_kernel<T><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k, ratio, grad);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
@@ -281,7 +285,7 @@ int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
 {
   {
     ProfScope ps(c, QMC_K_ACCEPT);
-    accept_kernel<T><<<c->dev.W, MOVE_NT, accept_smem(c->dev), c->stream>>>(c->dev, k, acc_out);
+    accept_kernel<T><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k, acc_out);
     LAUNCH_CHECK(c);
   }
   if (c->dev.kd == 1) {
@@ -300,14 +304,7 @@ int launch_flush(qmc_crowd* c, int spin)
   const int fcols = FINALIZE_NT / (d.kdp > 32 ? d.kdp / 32 : 1);
   dim3 fgrid((d.ns + fcols - 1) / fcols, d.W);
   const size_t fsm = (size_t)d.kdp * d.kdp * 8;
-  const size_t flush_smem = (size_t)FLUSH_DEPTH * (FLUSH_WARPS * FLUSH_STRIP_BYTES + (size_t)d.kdp * 128);
-  if (flush_smem > 48 * 1024 && !c->flush_attr_set) {
-    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
-    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
-    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
-    CUDA_TRY(cudaFuncSetAttribute(flush_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)flush_smem));
-    c->flush_attr_set = 1;
-  }
+  const size_t flush_smem = 0;
   switch (d.kdp) {
     case 8:
       flush_finalize_kernel<8><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
@@ -358,17 +355,54 @@ int step_accept(qmc_crowd* c, int k, unsigned char* acc)
 }
 
 // one full sweep, D:C6 flush schedule; no host synchronisation (capturable)
+template <typename T>
+int launch_fused_t(qmc_crowd* c, int k, bool next)
+{
+  ProfScope ps(c, next ? QMC_K_FUSED_MOVE : QMC_K_RATIO_ACCEPT);
+  const int mmax = c->dev.kd > 1 ? (k % c->dev.n) % c->dev.kd + 1 : 0;   // proposals of the open window incl. k
+  if (next) move_fused_kernel<T, true><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k, mmax);
+  else move_fused_kernel<T, false><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k, mmax);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
+// One full sweep with the D:C6 flush schedule; no host synchronisation (capturable).
+// Per move: spline(k), then ONE kernel doing ratio(k) + accept(k) + row/proposal of electron k+1;
+// the row/proposal is a kernel of its own only at k = 0 and after a rank-1 update or a flush
+// (it must see the updated inverse).
 int sweep_once(qmc_crowd* c)
 {
   const CrowdDev& d = c->dev;
+  int st = QMC_OK;
+  {
+    ProfScope ps(c, QMC_K_ROW_PROPOSE);
+    st = c->is_f64 ? launch_row_propose_t<double>(c, 0, nullptr) : launch_row_propose_t<float>(c, 0, nullptr);
+  }
+  if (st) return st;
   for (int k = 0; k < d.N; ++k) {
-    int st = step_vgl(c, k, nullptr);
-    if (!st) st = step_ratio(c, k, nullptr, nullptr);
-    if (!st) st = step_accept(c, k, nullptr);
+    {
+      ProfScope ps(c, QMC_K_SPLINE_VGL);
+      st = c->is_f64 ? launch_spline_t<double>(c) : launch_spline_t<float>(c);
+    }
     if (st) return st;
     const int kk = k % d.n;
-    if (d.kd > 1 && (((kk + 1) % d.kd) == 0 || kk == d.n - 1)) {
+    const bool flush_due = d.kd > 1 && (((kk + 1) % d.kd) == 0 || kk == d.n - 1);
+    const bool last = k == d.N - 1;
+    const bool fuse_next = d.kd > 1 && !flush_due && !last;
+    st = c->is_f64 ? launch_fused_t<double>(c, k, fuse_next) : launch_fused_t<float>(c, k, fuse_next);
+    if (st) return st;
+    if (d.kd == 1) {
+      ProfScope ps(c, QMC_K_RANK1);
+      st = c->is_f64 ? launch_rank1_t<double>(c, k) : launch_rank1_t<float>(c, k);
+      if (st) return st;
+    }
+    if (flush_due) {
       st = launch_flush(c, k / d.n);
+      if (st) return st;
+    }
+    if (!fuse_next && !last) {
+      ProfScope ps(c, QMC_K_ROW_PROPOSE);
+      st = c->is_f64 ? launch_row_propose_t<double>(c, k + 1, nullptr) : launch_row_propose_t<float>(c, k + 1, nullptr);
       if (st) return st;
     }
   }
@@ -430,7 +464,7 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   c->proposed = c->flushes = c->launches = 0;
   c->sweep_host = 0;
   c->use_graph = 1;
-  c->flush_attr_set = 0;
+  c->graph_launches = c->graph_flushes = 0;
   c->graph_exec = nullptr;
   c->profile = 0;
   c->ev_used = 0;
@@ -461,11 +495,17 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   e = cudaMemcpyAsync(d.R, pos_dev, (size_t)d.W * d.N * 3 * 8, cudaMemcpyDeviceToDevice, c->stream);
   if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "position copy: %s", cudaGetErrorString(e)));
   c->launches += 2;
-  if (row_smem(d) > 48 * 1024) {
-    e = cudaFuncSetAttribute(row_propose_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem(d));
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(row_propose_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)row_smem(d));
-    if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
+  if (move_smem(d) > 48 * 1024) {
+    const int sm = (int)move_smem(d);
+    const void* fns[] = {(const void*)row_propose_kernel<float>, (const void*)row_propose_kernel<double>,
+                         (const void*)ratio_grad_kernel<float>, (const void*)ratio_grad_kernel<double>,
+                         (const void*)accept_kernel<float>, (const void*)accept_kernel<double>,
+                         (const void*)move_fused_kernel<float, true>, (const void*)move_fused_kernel<float, false>,
+                         (const void*)move_fused_kernel<double, true>, (const void*)move_fused_kernel<double, false>};
+    for (const void* f : fns) {
+      e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+      if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
+    }
   }
   st = rebuild(c);
   if (st) return bail(st);
@@ -573,6 +613,8 @@ int qmc_sweep(qmc_crowd_t* c, int n_sweeps)
       c->stream = user;
       e = cudaStreamEndCapture(cap, &graph);
     }
+    c->graph_launches = c->launches - launches0;
+    c->graph_flushes = c->flushes - flushes0;
     c->launches = launches0;
     c->flushes = flushes0;
     if (st == QMC_OK && e == cudaSuccess) e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
@@ -582,13 +624,11 @@ int qmc_sweep(qmc_crowd_t* c, int n_sweeps)
     if (e != cudaSuccess) { c->graph_exec = nullptr; return fail(QMC_ERR_CUDA, "graph capture: %s", cudaGetErrorString(e)); }
   }
   const CrowdDev& d = c->dev;
-  // launches per sweep: 4 (+1 rank-1) per move, 3 per flush, 1 sweep bump
-  const uint64_t flushes_per_sweep = d.kd > 1 ? 2ull * ((d.n + d.kd - 1) / d.kd) : 0;
   for (int s = 0; s < n_sweeps; ++s) {
     if (c->use_graph && !c->profile) {
       CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
-      c->launches += (uint64_t)d.N * (d.kd == 1 ? 5 : 4) + 3 * flushes_per_sweep + 1;
-      c->flushes += flushes_per_sweep;
+      c->launches += c->graph_launches;
+      c->flushes += c->graph_flushes;
     } else {
       st = sweep_once(c);
       if (st) return st;

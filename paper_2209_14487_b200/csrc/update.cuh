@@ -156,113 +156,114 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d)
   }
 }
 
-// ---- operand streams of the strip kernel: a cp.async ring in shared memory ---------------------
-// Per 16-column chunk a CTA of 4 warps (64 strip rows) needs
-//   - per warp: 16 rows x 128 B of the B0 strip (GEMM-1 A fragments; again as GEMM-2 accumulator init),
-//   - per CTA:  the chunk of V (GEMM 1) or of Z (GEMM 2): kdp rows x 128 B, shared by the 4 warps.
-// The strip comes from DRAM and V/Z from L2; both latencies are far longer than one chunk of DMMAs,
-// so everything is streamed FLUSH_DEPTH-1 chunks ahead with 16-byte cp.async (each warp instruction
-// moves full 128-byte row segments) into a ring of stages.  Pieces are placed so that every fragment
-// read is one conflict-free LDS.128:
-//   strip piece (row r of block i, 16-byte column c)  -> [i][c & 1][4 r + c / 2]      (lane g = r, t = c / 2)
-//   V piece (window row l, column c)                  -> [l / 8][c & 1][4 (l % 8) + c / 2]
-//   Z piece (window row l, column c)                  -> [l / 8][l & 1][4 c + (l % 8) / 2]  (lane g = c, t = (l % 8) / 2)
-constexpr int FLUSH_DEPTH = 6;
-constexpr int FLUSH_WARPS = FLUSH_NT / 32;
-constexpr int FLUSH_STRIP_BYTES = 2 * 2 * 32 * 16;  // per warp and stage
+// ---- strip kernel: fragments straight from global memory, software-pipelined in registers -------
+// (A shared-memory cp.async ring for the operands was measured slower on B200: 2.54 ms vs 2.07 ms per
+// flush at cfg 5 / W = 2048 -- the LDS + LDGSTS instruction stream saturates the MIO queue next to
+// the DMMAs; see profiles/r1b_flush_variants.md.)
 
-__device__ __forceinline__ void cp_async16(unsigned smem_addr, const void* gptr)
-{
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
+// Fragment set of one 16-column chunk of GEMM 1: the B0 strip (two 8-row blocks) and KB window blocks of V.
 template <int KB>
-struct FlushStage {
-  static constexpr int VZ_BYTES = KB * 1024;                              // kdp rows x 128 B
-  static constexpr int BYTES = FLUSH_WARPS * FLUSH_STRIP_BYTES + VZ_BYTES;
+struct Frag1 {
+  double a0[4], a1[4], v[KB][4];
 };
-
-__device__ __forceinline__ void lds32(const unsigned char* p, double (&r)[4])
+template <int KB>
+__device__ __forceinline__ void load_frag1(Frag1<KB>& f, const double* a0p, const double* a1p, const double* vp,
+                                           int s, int ns, int m, int mb, int g)
 {
-  const double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 512);
-  r[0] = a.x; r[1] = a.y; r[2] = b.x; r[3] = b.y;
+  ld32(a0p + s, f.a0);
+  ld32(a1p + s, f.a1);
+#pragma unroll
+  for (int b = 0; b < KB; ++b) {
+    f.v[b][0] = f.v[b][1] = f.v[b][2] = f.v[b][3] = 0.0;
+    if (b < mb && 8 * b + g < m) ld32(vp + (size_t)(8 * b) * ns + s, f.v[b]);
+  }
+}
+template <int KB>
+__device__ __forceinline__ void mma_frag1(double (&acc)[2][KB][2], const Frag1<KB>& f, int mb)
+{
+  // k-step outermost: 2 KB independent accumulator chains between dependent DMMAs
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+#pragma unroll
+    for (int b = 0; b < KB; ++b)
+      if (b < mb) {
+        dmma884(acc[0][b], f.a0[q], f.v[b][q]);
+        dmma884(acc[1][b], f.a1[q], f.v[b][q]);
+      }
+}
+
+// Fragment set of one 16-column chunk of GEMM 2: the B0 strip chunk (accumulator init) and Z rows.
+template <int KB>
+struct Frag2 {
+  double x0[4], x1[4];
+  double2 z[KB][2];
+};
+template <int KB>
+__device__ __forceinline__ void load_frag2(Frag2<KB>& f, const double* a0p, const double* a1p, const double* zp,
+                                           int j0, int ns, int m, int mb, int t)
+{
+  ld32(a0p + j0, f.x0);
+  ld32(a1p + j0, f.x1);
+#pragma unroll
+  for (int b = 0; b < KB; ++b)
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      f.z[b][q] = make_double2(0.0, 0.0);
+      if (b < mb && 8 * b + 2 * t + q < m) f.z[b][q] = *reinterpret_cast<const double2*>(zp + (size_t)(8 * b + q) * ns + j0);
+    }
+}
+template <int KB>
+__device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double (&nw)[2][KB][2], int mb, double* o0,
+                                                double* o1)
+{
+  // even / odd columns of the chunk are separate tiles (a lane ends up with 4 consecutive columns);
+  // two accumulator sets (even / odd window blocks) give 8 independent DMMA chains, summed at the end
+  double de0[2] = {f.x0[0], f.x0[2]}, do0[2] = {f.x0[1], f.x0[3]};
+  double de1[2] = {f.x1[0], f.x1[2]}, do1[2] = {f.x1[1], f.x1[3]};
+  double ee0[2] = {0.0, 0.0}, eo0[2] = {0.0, 0.0}, ee1[2] = {0.0, 0.0}, eo1[2] = {0.0, 0.0};
+#pragma unroll
+  for (int q = 0; q < 2; ++q)
+#pragma unroll
+    for (int b = 0; b < KB; ++b)
+      if (b < mb) {
+        if (b & 1) {
+          dmma884(ee0, nw[0][b][q], f.z[b][q].x);
+          dmma884(eo0, nw[0][b][q], f.z[b][q].y);
+          dmma884(ee1, nw[1][b][q], f.z[b][q].x);
+          dmma884(eo1, nw[1][b][q], f.z[b][q].y);
+        } else {
+          dmma884(de0, nw[0][b][q], f.z[b][q].x);
+          dmma884(do0, nw[0][b][q], f.z[b][q].y);
+          dmma884(de1, nw[1][b][q], f.z[b][q].x);
+          dmma884(do1, nw[1][b][q], f.z[b][q].y);
+        }
+      }
+  *reinterpret_cast<double2*>(o0) = make_double2(de0[0] + ee0[0], do0[0] + eo0[0]);
+  *reinterpret_cast<double2*>(o0 + 2) = make_double2(de0[1] + ee0[1], do0[1] + eo0[1]);
+  *reinterpret_cast<double2*>(o1) = make_double2(de1[0] + ee1[0], do1[0] + eo1[0]);
+  *reinterpret_cast<double2*>(o1 + 2) = make_double2(de1[1] + ee1[1], do1[1] + eo1[1]);
 }
 
 // Flush, step 2: B_strip <- B0_strip - (B0_strip V^T - E) Z.  KB = kdp / 8. grid = (ceil(ns / 64), W).
-// dynamic smem: FLUSH_DEPTH * FlushStage<KB>::BYTES
 template <int KB>
 __global__ void __launch_bounds__(FLUSH_NT, 2) flush_kernel(CrowdDev d, int spin)
 {
-  extern __shared__ __align__(16) unsigned char ring[];
-  constexpr int STAGE = FlushStage<KB>::BYTES;
-  constexpr int NPV = (KB * 64 + FLUSH_NT - 1) / FLUSH_NT;  // V/Z pieces per thread and chunk
   const int w = blockIdx.y;
   const int m = d.mwin[w];
   if (m == 0) return;
-  const int ns = d.ns, kdp = d.kdp, nch = ns / 16;
+  const int ns = d.ns, kdp = d.kdp;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  const int row0 = (blockIdx.x * FLUSH_WARPS + warp) * FLUSH_ROWS_PER_WARP;
-  const bool strip_ok = row0 < ns;   // warps past the last strip still help with the V/Z copies and barriers
+  const int row0 = (blockIdx.x * (FLUSH_NT / 32) + warp) * FLUSH_ROWS_PER_WARP;
+  if (row0 >= ns) return;
   double* B = d.Binv + ((size_t)w * 2 + spin) * ns * ns;
   const int* rows = d.rows + (size_t)w * kdp;
   const int mb = (m + 7) >> 3;  // 8-wide blocks of the window that hold accepted moves
-  const unsigned ring_s = (unsigned)__cvta_generic_to_shared(ring);
-
-  // ---- per-thread copy plan (loop invariant): 4 strip pieces, NPV pieces of V / Z ----
-  const double* s_src[4];
-  unsigned s_dst[4];
-#pragma unroll
-  for (int i = 0; i < 2; ++i)
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-      const int p = 32 * j + lane, r = p >> 3, c16 = p & 7;
-      s_src[2 * i + j] = B + (size_t)((strip_ok ? row0 : 0) + 8 * i + r) * ns + 2 * c16;
-      s_dst[2 * i + j] = (unsigned)(warp * FLUSH_STRIP_BYTES + i * 1024 + (c16 & 1) * 512 + (r * 4 + (c16 >> 1)) * 16);
-    }
-  const double* v_src[NPV];
-  const double* z_src[NPV];
-  unsigned v_dst[NPV], z_dst[NPV];
-  bool vz_ok[NPV];
-#pragma unroll
-  for (int it = 0; it < NPV; ++it) {
-    const int p = it * FLUSH_NT + threadIdx.x;
-    const int l = p >> 3, c16 = p & 7, b = l >> 3, r = l & 7;
-    vz_ok[it] = p < KB * 64 && l < m;   // rows at or beyond m keep the zeros written below
-    v_src[it] = d.V + ((size_t)w * kdp + (vz_ok[it] ? l : 0)) * ns + 2 * c16;
-    z_src[it] = d.C + ((size_t)w * kdp + (vz_ok[it] ? l : 0)) * ns + 2 * c16;
-    v_dst[it] = (unsigned)(FLUSH_WARPS * FLUSH_STRIP_BYTES + b * 1024 + (c16 & 1) * 512 + (r * 4 + (c16 >> 1)) * 16);
-    z_dst[it] = (unsigned)(FLUSH_WARPS * FLUSH_STRIP_BYTES + b * 1024 + (r & 1) * 512 + (c16 * 4 + (r >> 1)) * 16);
-  }
-  // zero the ring once: window rows >= m are never copied, so their V slots read as 0 (their Z slots
-  // may later hold stale finite V data, which only ever multiplies the exact zeros of nw)
-  for (int e = threadIdx.x; e < FLUSH_DEPTH * STAGE / 16; e += FLUSH_NT)
-    *reinterpret_cast<double2*>(ring + (size_t)e * 16) = make_double2(0.0, 0.0);
-  __syncthreads();
-
-  // seq q in [0, 2 nch): chunk q mod nch; first pass carries V (GEMM 1), second pass Z (GEMM 2)
-  auto issue = [&](int q, unsigned st) {
-    if (q < 2 * nch) {
-      const bool first = q < nch;
-      const int off = 16 * (first ? q : q - nch);
-      if (strip_ok) {
-#pragma unroll
-        for (int e = 0; e < 4; ++e) cp_async16(ring_s + st + s_dst[e], s_src[e] + off);
-      }
-#pragma unroll
-      for (int it = 0; it < NPV; ++it)
-        if (vz_ok[it]) cp_async16(ring_s + st + (first ? v_dst[it] : z_dst[it]), (first ? v_src[it] : z_src[it]) + off);
-    }
-    cp_async_commit();  // always, so that group counting stays uniform
-  };
-#pragma unroll
-  for (int q = 0; q < FLUSH_DEPTH - 1; ++q) issue(q, (unsigned)(q * STAGE));
-
-  const unsigned char* my_strip = ring + warp * FLUSH_STRIP_BYTES + lane * 16;
-  const unsigned char* my_vz = ring + FLUSH_WARPS * FLUSH_STRIP_BYTES + lane * 16;
-  unsigned st_rd = 0, st_wr = (FLUSH_DEPTH - 1) * STAGE;   // stage being consumed / refilled
+  double* a0p = B + (size_t)(row0 + g) * ns + 4 * t;
+  double* a1p = a0p + (size_t)8 * ns;
+  // lane's V fragment base: row g of each window block, columns 4t..4t+3 of the chunk
+  const double* vp = d.V + (size_t)w * kdp * ns + (size_t)g * ns + 4 * t;
+  // lane's Z fragment base: rows 2t (+q) of each window block, columns 2g, 2g+1 of the chunk
+  const double* zp = d.C + (size_t)w * kdp * ns + (size_t)(2 * t) * ns + 2 * g;
 
   // GEMM 1: Wm = B0_strip V^T. acc[i][b] = tile (rows row0+8i.., window columns 8b..8b+7);
   // lane holds (row g, columns 8b+2t, 8b+2t+1).
@@ -271,29 +272,17 @@ __global__ void __launch_bounds__(FLUSH_NT, 2) flush_kernel(CrowdDev d, int spin
   for (int i = 0; i < 2; ++i)
 #pragma unroll
     for (int b = 0; b < KB; ++b) acc[i][b][0] = acc[i][b][1] = 0.0;
-  for (int q = 0; q < nch; ++q) {
-    cp_async_wait<FLUSH_DEPTH - 2>();
-    __syncthreads();   // stage q landed for everyone; everyone is done reading stage q-1
-    issue(q + FLUSH_DEPTH - 1, st_wr);
-    if (strip_ok) {
-      double a0[4], a1[4], v[KB][4];
-      lds32(my_strip + st_rd, a0);
-      lds32(my_strip + st_rd + 1024, a1);
-#pragma unroll
-      for (int b = 0; b < KB; ++b)
-        if (b < mb) lds32(my_vz + st_rd + b * 1024, v[b]);
-      // k-step outermost: 2 KB independent accumulator chains between dependent DMMAs
-#pragma unroll
-      for (int kq = 0; kq < 4; ++kq)
-#pragma unroll
-        for (int b = 0; b < KB; ++b)
-          if (b < mb) {
-            dmma884(acc[0][b], a0[kq], v[b][kq]);
-            dmma884(acc[1][b], a1[kq], v[b][kq]);
-          }
+  {
+    Frag1<KB> fa, fb;
+    load_frag1<KB>(fa, a0p, a1p, vp, 0, ns, m, mb, g);
+    for (int s = 0; s < ns; s += 32) {
+      if (s + 16 < ns) load_frag1<KB>(fb, a0p, a1p, vp, s + 16, ns, m, mb, g);
+      mma_frag1<KB>(acc, fa, mb);
+      if (s + 16 < ns) {
+        if (s + 32 < ns) load_frag1<KB>(fa, a0p, a1p, vp, s + 32, ns, m, mb, g);
+        mma_frag1<KB>(acc, fb, mb);
+      }
     }
-    st_rd = st_rd + STAGE == FLUSH_DEPTH * STAGE ? 0u : st_rd + STAGE;
-    st_wr = st_wr + STAGE == FLUSH_DEPTH * STAGE ? 0u : st_wr + STAGE;
   }
   // minus E (E[rows[l]][l] = 1), then negate: nw = -(B0 V^T - E)
 #pragma unroll
@@ -308,55 +297,19 @@ __global__ void __launch_bounds__(FLUSH_NT, 2) flush_kernel(CrowdDev d, int spin
       }
     }
   }
-  // GEMM 2: B_strip = B0_strip + nw Z, 16 columns at a time.  Even / odd columns of the chunk are
-  // separate tiles (a lane ends up with 4 consecutive columns); two accumulator sets (even / odd
-  // window blocks) give 8 independent DMMA chains, summed at the end.
-  double* o0 = B + (size_t)(row0 + g) * ns + 4 * t;   // the same 32 bytes per row the lane took as accumulators
-  double* o1 = o0 + (size_t)8 * ns;
-  for (int c = 0; c < nch; ++c) {
-    cp_async_wait<FLUSH_DEPTH - 2>();
-    __syncthreads();
-    issue(nch + c + FLUSH_DEPTH - 1, st_wr);
-    if (strip_ok) {
-      double x0[4], x1[4];
-      double2 z[KB][2];
-      lds32(my_strip + st_rd, x0);
-      lds32(my_strip + st_rd + 1024, x1);
-#pragma unroll
-      for (int b = 0; b < KB; ++b)
-        if (b < mb) {
-          z[b][0] = *reinterpret_cast<const double2*>(my_vz + st_rd + b * 1024);
-          z[b][1] = *reinterpret_cast<const double2*>(my_vz + st_rd + b * 1024 + 512);
-        }
-      double de0[2] = {x0[0], x0[2]}, do0[2] = {x0[1], x0[3]};
-      double de1[2] = {x1[0], x1[2]}, do1[2] = {x1[1], x1[3]};
-      double ee0[2] = {0.0, 0.0}, eo0[2] = {0.0, 0.0}, ee1[2] = {0.0, 0.0}, eo1[2] = {0.0, 0.0};
-#pragma unroll
-      for (int kq = 0; kq < 2; ++kq)
-#pragma unroll
-        for (int b = 0; b < KB; ++b)
-          if (b < mb) {
-            if (b & 1) {
-              dmma884(ee0, acc[0][b][kq], z[b][kq].x);
-              dmma884(eo0, acc[0][b][kq], z[b][kq].y);
-              dmma884(ee1, acc[1][b][kq], z[b][kq].x);
-              dmma884(eo1, acc[1][b][kq], z[b][kq].y);
-            } else {
-              dmma884(de0, acc[0][b][kq], z[b][kq].x);
-              dmma884(do0, acc[0][b][kq], z[b][kq].y);
-              dmma884(de1, acc[1][b][kq], z[b][kq].x);
-              dmma884(do1, acc[1][b][kq], z[b][kq].y);
-            }
-          }
-      *reinterpret_cast<double2*>(o0 + 16 * c) = make_double2(de0[0] + ee0[0], do0[0] + eo0[0]);
-      *reinterpret_cast<double2*>(o0 + 16 * c + 2) = make_double2(de0[1] + ee0[1], do0[1] + eo0[1]);
-      *reinterpret_cast<double2*>(o1 + 16 * c) = make_double2(de1[0] + ee1[0], do1[0] + eo1[0]);
-      *reinterpret_cast<double2*>(o1 + 16 * c + 2) = make_double2(de1[1] + ee1[1], do1[1] + eo1[1]);
+  // GEMM 2: B_strip = B0_strip + nw Z, 16 columns at a time
+  {
+    Frag2<KB> fa, fb;
+    load_frag2<KB>(fa, a0p, a1p, zp, 0, ns, m, mb, t);
+    for (int j0 = 0; j0 < ns; j0 += 32) {
+      if (j0 + 16 < ns) load_frag2<KB>(fb, a0p, a1p, zp, j0 + 16, ns, m, mb, t);
+      mma_store_frag2<KB>(fa, acc, mb, a0p + j0, a1p + j0);
+      if (j0 + 16 < ns) {
+        if (j0 + 32 < ns) load_frag2<KB>(fa, a0p, a1p, zp, j0 + 32, ns, m, mb, t);
+        mma_store_frag2<KB>(fb, acc, mb, a0p + j0 + 16, a1p + j0 + 16);
+      }
     }
-    st_rd = st_rd + STAGE == FLUSH_DEPTH * STAGE ? 0u : st_rd + STAGE;
-    st_wr = st_wr + STAGE == FLUSH_DEPTH * STAGE ? 0u : st_wr + STAGE;
   }
-  cp_async_wait<0>();
 }
 
 }  // namespace qmc

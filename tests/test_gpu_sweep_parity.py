@@ -84,6 +84,31 @@ def test_graph_replay_equals_plain_launches_and_crowd_split(kd):
     assert not np.array_equal(Ra, pos)
 
 
+@pytest.mark.parametrize("n_elec,kd", [(48, 8), (40, 16), (24, 1)])
+def test_sweep_equals_the_three_step_calls(n_elec, kd):
+    """qmc_sweep runs fused kernels (ratio + accept + next row in one launch); the step calls run the
+    same device functions one per launch.  Both must give bit-identical trajectories."""
+    wl = qi.small_workload(n_elec=n_elec, grid=10, box=6.0, coef_dtype="f32", coef_dist="normal", n_walkers=7,
+                           tau=0.02, delay_rank=kd, cfg=14)
+    a, _, _, _ = make_pair(wl)
+    b, _, _, _ = make_pair(wl)
+    n = n_elec // 2
+    for s in range(2):
+        a.qmc_sweep(1)
+        b.set_sweep_index(s)
+        for k in range(n_elec):
+            b.qmc_spo_vgl(k)
+            b.qmc_ratio_grad(k)
+            b.qmc_accept_reject(k)
+            kk = k % n
+            if kd > 1 and ((kk + 1) % kd == 0 or kk == n - 1):
+                b.qmc_flush_delayed()
+        assert np.array_equal(npy(a.positions()), npy(b.positions()))
+        for spin in (0, 1):
+            assert np.array_equal(npy(a.inverse(spin)), npy(b.inverse(spin)))
+    assert a.stats() == b.stats()
+
+
 def _gpu_slater(crowd, R, spin):
     """A[w][i][j] = phi_j(r_{spin n + i}) from the CUDA spline at given positions (teacher-forced)."""
     import torch
