@@ -101,6 +101,197 @@ __global__ void __launch_bounds__(INV_NT) invert_kernel(CrowdDev d)
   }
 }
 
+// ---- blocked variant (the one qmc_crowd_create uses when its shared memory fits) -----------------
+// Same elimination, same pivot choices, but right-looking in panels of INVB_NB columns so that the
+// matrix is swept 2 n / NB times instead of 2 n times (the unblocked kernel is bound by that
+// traffic: 3.7 TB at cfg 5 / W = 4096):
+//   (a) the panel (n x NB) is loaded into shared memory and eliminated there, unblocked, in place:
+//       afterwards it holds the NB columns X_G of the composite Gauss-Jordan operator G of the panel;
+//   (b) the panel's row swaps are applied to all other columns (column-local, no barrier);
+//   (c) the pivot rows A_K (NB x n) are copied to shared memory;
+//   (d) every other column block is updated with one FP64 tensor-core GEMM,
+//       A[:, o] <- A[:, o] + (X_G - E_K) A_K[:, o]   (rows of K: A[K, o] <- X_G[K, :] A_K[:, o]),
+//       32 x 32 register tiles per warp, fragments read conflict-free from padded shared memory.
+constexpr int INVB_NT = 512;
+constexpr int INVB_NB = 32;
+constexpr int INVB_XS = INVB_NB + 4;   // row stride of the panel in smem (doubles): 4 g + t bank pattern
+
+inline __host__ __device__ size_t invert_blocked_smem(int ns)
+{
+  return ((size_t)ns * INVB_XS + (size_t)INVB_NB * (ns + 4) + ns + INVB_NB + 2 * (INVB_NT / 32)) * 8 + (size_t)ns * 4 + 64;
+}
+
+__global__ void __launch_bounds__(INVB_NT) invert_blocked_kernel(CrowdDev d)
+{
+  extern __shared__ double sm[];
+  const int ns = d.ns, n = d.n, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int as = ns + 4;                       // row stride of A_K
+  double* XG = sm;                             // [ns][INVB_XS]
+  double* AK = XG + (size_t)ns * INVB_XS;      // [NB][ns + 4]
+  double* colf = AK + (size_t)INVB_NB * as;    // [ns]
+  double* rowc = colf + ns;                    // [NB]
+  double* redv = rowc + INVB_NB;
+  int* redi = reinterpret_cast<int*>(redv + INVB_NT / 32);
+  int* piv = redi + INVB_NT / 32;
+  __shared__ int s_p;
+  __shared__ int s_bad;
+  double* X = d.Binv + (size_t)blockIdx.x * ns * ns;
+  if (tid == 0) s_bad = 0;
+  __syncthreads();
+  for (int c0 = 0; c0 < n; c0 += INVB_NB) {
+    const int nb = min(INVB_NB, n - c0);
+    // (a) panel into shared memory (zero padded), then unblocked in-place Gauss-Jordan on it
+    for (int e = tid; e < ns * INVB_NB; e += INVB_NT) {
+      const int r = e / INVB_NB, j = e - r * INVB_NB;
+      XG[r * INVB_XS + j] = (r < n && j < nb) ? X[(size_t)r * ns + c0 + j] : 0.0;
+    }
+    __syncthreads();
+    for (int j = 0; j < nb; ++j) {
+      const int c = c0 + j;
+      double best = -1.0;
+      int bi = c;
+      for (int r = c + tid; r < n; r += INVB_NT) {
+        double v = fabs(XG[r * INVB_XS + j]);
+        if (!(v == v)) v = INFINITY;
+        if (v > best) { best = v; bi = r; }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+      }
+      if (lane == 0) { redv[warp] = best; redi[warp] = bi; }
+      __syncthreads();
+      if (tid == 0) {
+        double bv = redv[0];
+        int bj = redi[0];
+        for (int q = 1; q < INVB_NT / 32; ++q)
+          if (redv[q] > bv || (redv[q] == bv && redi[q] < bj)) { bv = redv[q]; bj = redi[q]; }
+        s_p = bj;
+        piv[c] = bj;
+        if (!(bv > 0.0) || !isfinite(bv)) s_bad = 1;
+      }
+      __syncthreads();
+      if (s_bad) break;
+      const int p = s_p;
+      if (p != c) {
+        if (tid < INVB_NB) {
+          const double a = XG[c * INVB_XS + tid], b = XG[p * INVB_XS + tid];
+          XG[c * INVB_XS + tid] = b;
+          XG[p * INVB_XS + tid] = a;
+        }
+        __syncthreads();
+      }
+      const double pv = XG[c * INVB_XS + j];
+      for (int r = tid; r < n; r += INVB_NT) colf[r] = XG[r * INVB_XS + j];
+      if (tid < nb) rowc[tid] = (tid == j) ? 1.0 / pv : XG[c * INVB_XS + tid] / pv;   // true divisions (see above)
+      __syncthreads();
+      for (int e = tid; e < n * nb; e += INVB_NT) {
+        const int r = e / nb, jj = e - r * nb;
+        double v;
+        if (r == c) v = rowc[jj];
+        else v = fma(-colf[r], rowc[jj], (jj == j) ? 0.0 : XG[r * INVB_XS + jj]);
+        XG[r * INVB_XS + jj] = v;
+      }
+      __syncthreads();
+    }
+    if (s_bad) break;
+    // (b) the panel's row swaps on every other column (a thread owns whole columns: no barrier needed)
+    for (int o = tid; o < n; o += INVB_NT) {
+      if (o >= c0 && o < c0 + nb) continue;
+      for (int j = 0; j < nb; ++j) {
+        const int c = c0 + j, p = piv[c];
+        if (p != c) {
+          const double a = X[(size_t)c * ns + o], b = X[(size_t)p * ns + o];
+          X[(size_t)c * ns + o] = b;
+          X[(size_t)p * ns + o] = a;
+        }
+      }
+    }
+    __syncthreads();
+    // (c) pivot rows A_K (zero padded; the panel's own columns are not used)
+    for (int e = tid; e < INVB_NB * ns; e += INVB_NT) {
+      const int j = e / ns, o = e - j * ns;
+      AK[j * as + o] = (j < nb && o < n) ? X[(size_t)(c0 + j) * ns + o] : 0.0;
+    }
+    __syncthreads();
+    // (d) GEMM update, one 32 x 32 tile per warp at a time
+    {
+      const int g = lane >> 2, t = lane & 3;
+      const int nt = (n + 31) / 32;
+      for (int tile = warp; tile < nt * nt; tile += INVB_NT / 32) {
+        const int r0 = (tile / nt) * 32, o0 = (tile - (tile / nt) * nt) * 32;
+        if (o0 == c0) continue;                      // the panel's own columns come from XG
+        const bool in_k = r0 == c0;
+        double acc[4][4][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) {
+            const int r = r0 + 8 * i + g, o = o0 + 8 * b + 2 * t;
+            double2 x = make_double2(0.0, 0.0);
+            if (!in_k && r < n && o < ns) x = *reinterpret_cast<const double2*>(X + (size_t)r * ns + o);
+            acc[i][b][0] = x.x;
+            acc[i][b][1] = x.y;
+          }
+#pragma unroll
+        for (int ks = 0; ks < INVB_NB; ks += 4) {
+          double a[4], bb[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) a[i] = (r0 + 8 * i + g < ns) ? XG[(r0 + 8 * i + g) * INVB_XS + ks + t] : 0.0;
+#pragma unroll
+          for (int b = 0; b < 4; ++b) bb[b] = (o0 + 8 * b + g < ns) ? AK[(ks + t) * as + o0 + 8 * b + g] : 0.0;
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) dmma884(acc[i][b], a[i], bb[b]);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) {
+            const int r = r0 + 8 * i + g, o = o0 + 8 * b + 2 * t;
+            if (r < n) {
+              if (o < n) X[(size_t)r * ns + o] = acc[i][b][0];
+              if (o + 1 < n) X[(size_t)r * ns + o + 1] = acc[i][b][1];
+            }
+          }
+      }
+    }
+    // the panel's own columns
+    for (int e = tid; e < n * nb; e += INVB_NT) {
+      const int r = e / nb, j = e - r * nb;
+      X[(size_t)r * ns + c0 + j] = XG[r * INVB_XS + j];
+    }
+    __syncthreads();
+  }
+  if (s_bad) {
+    if (tid == 0) atomicExch(d.status, 4);
+    return;
+  }
+  // undo the row swaps as column swaps, last first: the swaps act on column labels, so run them on an
+  // index array once and then permute every row through shared memory (coalesced)
+  int* src = reinterpret_cast<int*>(colf);     // [n] final column j <- current column src[j]
+  for (int j = tid; j < n; j += INVB_NT) src[j] = j;
+  __syncthreads();
+  if (tid == 0)
+    for (int c = n - 1; c >= 0; --c) {
+      const int p = piv[c];
+      const int a = src[c];
+      src[c] = src[p];
+      src[p] = a;
+    }
+  __syncthreads();
+  double* rowbuf = AK + (size_t)warp * ns;     // one row per warp
+  for (int r = warp; r < n; r += INVB_NT / 32) {
+    for (int j = lane; j < n; j += 32) rowbuf[j] = X[(size_t)r * ns + j];
+    __syncwarp();
+    for (int j = lane; j < n; j += 32) X[(size_t)r * ns + j] = rowbuf[src[j]];
+    __syncwarp();
+  }
+}
+
 // dst[(b * rows + r) * cols + c] = src[b * sb + r * sr + c]   (gather = pack; scatter = unpack)
 template <typename TD, typename TS>
 __global__ void pack_kernel(TD* __restrict__ dst, const TS* __restrict__ src, size_t nb, int rows, int cols, size_t sb,

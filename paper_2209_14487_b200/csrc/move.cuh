@@ -13,9 +13,6 @@ namespace qmc {
 #ifndef QMC_MOVE_DOT_ROWS
 #define QMC_MOVE_DOT_ROWS 2
 #endif
-#ifndef QMC_MOVE_PREFETCH
-#define QMC_MOVE_PREFETCH 0
-#endif
 constexpr int MOVE_NT = QMC_MOVE_NT;
 constexpr int MOVE_RED = 8 * (MOVE_NT / 32) < 32 ? 32 : 8 * (MOVE_NT / 32);  // doubles of reduction scratch
 
@@ -342,33 +339,11 @@ __global__ void __launch_bounds__(MOVE_NT) accept_kernel(CrowdDev d, int k, unsi
   dev_accept<T>(d, blockIdx.x, k, acc_out, sm);
 }
 // ratio(k) + accept(k); with NEXT also row_propose(k + 1) (same spin block, no flush in between)
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-
-// mmax = upper bound of the window fill after this move (proposals of the open window incl. k)
 template <typename T, bool NEXT>
-__global__ void __launch_bounds__(MOVE_NT) move_fused_kernel(CrowdDev d, int k, int mmax)
+__global__ void __launch_bounds__(MOVE_NT) move_fused_kernel(CrowdDev d, int k)
 {
   extern __shared__ double sm[];
   const int w = blockIdx.x;
-  if (NEXT && QMC_MOVE_PREFETCH) {
-    // The CTA is a chain of short dependent phases, each a DRAM round trip.  Everything the later
-    // phases will read is known now: pull it into L2 while the ratio phase runs (no registers held).
-    const int ns = d.ns, lpr = ns / 16;              // 128-byte lines per fp64 row
-    const int spin = k / d.n, kk = k - spin * d.n;
-    const char* V = reinterpret_cast<const char*>(d.V + (size_t)w * d.kdp * ns);
-    const char* C = reinterpret_cast<const char*>(d.C + (size_t)w * d.kdp * ns);
-    const int nl = mmax * lpr;
-    for (int e = threadIdx.x; e < nl; e += MOVE_NT) {
-      prefetch_l2(V + (size_t)e * 128);
-      prefetch_l2(C + (size_t)e * 128);
-    }
-    const char* b0 = reinterpret_cast<const char*>(d.Binv + (((size_t)w * 2 + spin) * ns + kk) * ns);
-    const char* cache = static_cast<const char*>(d.cache) + ((size_t)w * d.N + k + 1) * 4 * ns * sizeof(T);
-    for (int e = threadIdx.x; e < 2 * lpr; e += MOVE_NT) prefetch_l2(b0 + (size_t)e * 128);   // rows kk and kk+1
-    for (int e = threadIdx.x; e < (int)(3 * ns * sizeof(T) / 128); e += MOVE_NT) prefetch_l2(cache + (size_t)e * 128);
-    const char* sinv = reinterpret_cast<const char*>(d.Sinv + (size_t)w * d.kdp * d.kdp);
-    for (int e = threadIdx.x; e < mmax * d.kdp / 16; e += MOVE_NT) prefetch_l2(sinv + (size_t)e * 128);
-  }
   dev_ratio_grad<T>(d, w, k, nullptr, nullptr, sm);
   __syncthreads();
   dev_accept<T>(d, w, k, nullptr, sm);

@@ -213,9 +213,15 @@ int rebuild(qmc_crowd* c)
   c->launches += 3;
   int st = c->is_f64 ? launch_build_t<double>(c) : launch_build_t<float>(c);
   if (st) return st;
-  const size_t smem = (size_t)(2 * d.ns + 2 * (INV_NT / 32)) * 8 + (size_t)d.ns * 4 + 64;
-  if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  invert_kernel<<<(unsigned)(d.W * 2), INV_NT, smem, c->stream>>>(d);
+  const size_t bsmem = invert_blocked_smem(d.ns);
+  if (bsmem <= 227 * 1024) {
+    if (bsmem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_blocked_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsmem));
+    invert_blocked_kernel<<<(unsigned)(d.W * 2), INVB_NT, bsmem, c->stream>>>(d);
+  } else {
+    const size_t smem = (size_t)(2 * d.ns + 2 * (INV_NT / 32)) * 8 + (size_t)d.ns * 4 + 64;
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    invert_kernel<<<(unsigned)(d.W * 2), INV_NT, smem, c->stream>>>(d);
+  }
   LAUNCH_CHECK(c);
   int status = 0;
   CUDA_TRY(cudaMemcpyAsync(&status, d.status, 4, cudaMemcpyDeviceToHost, c->stream));
@@ -359,9 +365,8 @@ template <typename T>
 int launch_fused_t(qmc_crowd* c, int k, bool next)
 {
   ProfScope ps(c, next ? QMC_K_FUSED_MOVE : QMC_K_RATIO_ACCEPT);
-  const int mmax = c->dev.kd > 1 ? (k % c->dev.n) % c->dev.kd + 1 : 0;   // proposals of the open window incl. k
-  if (next) move_fused_kernel<T, true><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k, mmax);
-  else move_fused_kernel<T, false><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k, mmax);
+  if (next) move_fused_kernel<T, true><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k);
+  else move_fused_kernel<T, false><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
