@@ -177,6 +177,10 @@ def algorithmic(wl, W, kd, alpha, el):
         "ratio_accept": {"bytes": ratio_b + accept_b},
         # fused ratio(k) + accept(k) + row(k+1): C rows and positions are needed once, not twice
         "fused_move": {"bytes": ratio_b + accept_b + row_b - alpha * W * 8 * n * m_move - W * 24 * N},
+        # one launch = all kd moves of a delay window: spline + ratio + accept + row per move
+        "window": {"bytes": kd * (W * (64 * M * el + 5 * M * el) + ratio_b + accept_b + row_b
+                                  - alpha * W * 8 * n * m_move - W * 24 * N),
+                   "flops": kd * W * 600 * M},
         "rank1": {"bytes": alpha * W * 16 * n * n, "flops": alpha * W * 4 * n * n},
         "flush": {"bytes": W * 16 * n * n, "flops": W * (4 * n * n * m_flush + 2 * n * m_flush ** 2)},
     }

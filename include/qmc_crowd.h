@@ -171,7 +171,8 @@ enum {
   QMC_K_FLUSH = 5,       /* delayed rank-k flush, FP64 DMMA (step a5)                            */
   QMC_K_RATIO_ACCEPT = 6,/* qmc_sweep only: ratio_grad + accept of electron k in one kernel      */
   QMC_K_FUSED_MOVE = 7,  /* qmc_sweep only: ratio_grad + accept of k, row/proposal of k+1        */
-  QMC_N_KERNEL_CLASSES = 8
+  QMC_K_WINDOW = 8,      /* qmc_sweep, delay_rank > 1: all moves of one delay window, CTA per walker */
+  QMC_N_KERNEL_CLASSES = 9
 };
 /* Device time (ms, CUDA events on desc.stream) and launch count per kernel class accumulated in
  * profile mode since the previous call; resets the accumulators.  Synchronous.  ms and count

@@ -17,7 +17,7 @@ QMC_OK, QMC_ERR_INVALID_ARG, QMC_ERR_CUDA, QMC_ERR_WORKSPACE, QMC_ERR_SINGULAR, 
 QMC_OPT_GRAPH = 0
 QMC_OPT_PROFILE = 1
 KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush", "ratio_accept",
-                  "fused_move")
+                  "fused_move", "window")
 
 EXPORTS = [
     "qmc_crowd_workspace_bytes", "qmc_crowd_create", "qmc_crowd_destroy", "qmc_spo_vgl", "qmc_ratio_grad",

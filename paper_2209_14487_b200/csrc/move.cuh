@@ -4,6 +4,7 @@
 // length-n / length-N sums are strided over the block and combined by shuffle reductions (BJ).
 #pragma once
 #include "common.cuh"
+#include "spline.cuh"
 
 namespace qmc {
 
@@ -18,7 +19,7 @@ constexpr int MOVE_RED = 8 * (MOVE_NT / 32) < 32 ? 32 : 8 * (MOVE_NT / 32);  // 
 
 // D:C3: one pair term of the two-body Jastrow for electron k placed at rk against electron i.
 // u(r) = a r/(1 + b r), u'(r) = a/(1 + b r)^2, minimum image d_c <- d_c - L rint(d_c/L).
-__device__ __forceinline__ void j2_pair(const CrowdDev& d, const double (&rk)[3], const double* __restrict__ ri,
+__device__ __forceinline__ void j2_pair(const CrowdDev& d, const double (&rk)[3], const double* ri,
                                         double& usum, double (&g)[3])
 {
   double dd[3], r2 = 0.0;
@@ -45,7 +46,7 @@ __device__ __forceinline__ void j2_pair(const CrowdDev& d, const double (&rk)[3]
 // (one DRAM round trip per group instead of one per row); then shuffle-reduces each row.
 constexpr int MOVE_DOT_ROWS = QMC_MOVE_DOT_ROWS;
 template <typename F>
-__device__ __forceinline__ void rows_dot(const double* __restrict__ mat, int ns, int nrows, const double* x_s, F&& store)
+__device__ __forceinline__ void rows_dot(const double* mat, int ns, int nrows, const double* x_s, F&& store)
 {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int l0 = warp * MOVE_DOT_ROWS; l0 < nrows; l0 += (MOVE_NT / 32) * MOVE_DOT_ROWS) {
@@ -350,6 +351,44 @@ __global__ void __launch_bounds__(MOVE_NT) move_fused_kernel(CrowdDev d, int k)
   if (NEXT) {
     __syncthreads();
     dev_row_propose<T>(d, w, k + 1, nullptr, sm);
+  }
+}
+
+// ---- qmc_sweep, delayed update: one launch per delay window ---------------------------------------
+// The crowd advances in lock-step per *window*: a CTA owns one walker for the cnt <= delay_rank
+// moves k0 .. k0+cnt-1 of the window (row/proposal, spline, ratio, accept, append for each), then the
+// whole crowd flushes.  Walkers never interact inside a window, so nothing needs a kernel boundary
+// between moves: the SM overlaps the DRAM-bound gather of one walker with the fp64 work of the others,
+// the window rows V, C a walker appends stay in L2 for its next moves, and the launch tail is paid
+// once per window instead of twice per move.  Same device functions as the step kernels.
+// dynamic smem: move_smem_doubles(d) doubles
+template <typename T>
+__global__ void __launch_bounds__(MOVE_NT, 4) window_kernel(CrowdDev d, int k0, int cnt)
+{
+  extern __shared__ double sm[];
+  __shared__ SplineW<T> sw;
+  const int w = blockIdx.x, ns = d.ns;
+  T* vgl = static_cast<T*>(d.vgl) + (size_t)w * 5 * ns;
+  const int spin = k0 / d.n;
+  for (int k = k0; k < k0 + cnt; ++k) {
+    if (k + 1 < k0 + cnt) {
+      // next move's inverse row and gradient cache are first-touch DRAM lines: pull them into L2 now
+      const int kk1 = k + 1 - spin * d.n;
+      const char* brow_n = reinterpret_cast<const char*>(d.Binv + (((size_t)w * 2 + spin) * ns + kk1) * ns);
+      const char* cache_n = reinterpret_cast<const char*>(static_cast<const T*>(d.cache) + ((size_t)w * d.N + k + 1) * 4 * ns);
+      const int lb = ns * 8 / 128, lc = 3 * ns * (int)sizeof(T) / 128;
+      for (int i = threadIdx.x; i < lb + lc; i += MOVE_NT) {
+        const char* p = i < lb ? brow_n + (size_t)i * 128 : cache_n + (size_t)(i - lb) * 128;
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+      }
+    }
+    dev_row_propose<T>(d, w, k, nullptr, sm);
+    spline_cta<T, MOVE_NT>(d, d.rnew + 3 * (size_t)w, sw, vgl);
+    __syncthreads();
+    dev_ratio_grad<T>(d, w, k, nullptr, nullptr, sm);
+    __syncthreads();
+    dev_accept<T>(d, w, k, nullptr, sm);
+    __syncthreads();
   }
 }
 

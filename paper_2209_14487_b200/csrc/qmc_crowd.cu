@@ -194,11 +194,11 @@ template <typename T>
 int launch_build_t(qmc_crowd* c)
 {
   const CrowdDev& d = c->dev;
-  const size_t chunks = (size_t)d.ns / Vec16<T>::W;
-  const size_t items = (size_t)d.W * d.N * chunks;
-  const size_t blocks = (items + SPLINE_NT - 1) / SPLINE_NT;
+  const size_t blocks = (size_t)d.W * d.N;
   if (blocks > 0x7fffffffull) return fail(QMC_ERR_INVALID_ARG, "crowd too large for one build launch");
-  spline_build_kernel<T><<<(unsigned)blocks, SPLINE_NT, 0, c->stream>>>(d);
+  const size_t smem = (size_t)5 * d.ns * sizeof(T);
+  if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(spline_build_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  spline_build_kernel<T><<<(unsigned)blocks, SPLINE_NT, smem, c->stream>>>(d);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
@@ -252,8 +252,7 @@ template <typename T>
 int launch_spline_t(qmc_crowd* c)
 {
   const CrowdDev& d = c->dev;
-  const size_t items = (size_t)d.W * (d.ns / Vec16<T>::W);
-  spline_vgl_kernel<T><<<(unsigned)((items + SPLINE_NT - 1) / SPLINE_NT), SPLINE_NT, 0, c->stream>>>(d);
+  spline_vgl_kernel<T><<<(unsigned)d.W, SPLINE_NT, 0, c->stream>>>(d);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
@@ -371,14 +370,36 @@ int launch_fused_t(qmc_crowd* c, int k, bool next)
   return QMC_OK;
 }
 
+template <typename T>
+int launch_window_t(qmc_crowd* c, int k0, int cnt)
+{
+  ProfScope ps(c, QMC_K_WINDOW);
+  window_kernel<T><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k0, cnt);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+
 // One full sweep with the D:C6 flush schedule; no host synchronisation (capturable).
-// Per move: spline(k), then ONE kernel doing ratio(k) + accept(k) + row/proposal of electron k+1;
-// the row/proposal is a kernel of its own only at k = 0 and after a rank-1 update or a flush
-// (it must see the updated inverse).
+// delay_rank > 1: per delay window ONE walker-persistent kernel (all moves of the window) + the flush.
+// delay_rank = 1: per move spline(k), ratio(k) + accept(k), the rank-1 update, row/proposal of k+1
+// (which must see the updated inverse).
 int sweep_once(qmc_crowd* c)
 {
   const CrowdDev& d = c->dev;
   int st = QMC_OK;
+  if (d.kd > 1) {
+    for (int spin = 0; spin < 2; ++spin)
+      for (int kk0 = 0; kk0 < d.n; kk0 += d.kd) {
+        const int cnt = d.n - kk0 < d.kd ? d.n - kk0 : d.kd;
+        st = c->is_f64 ? launch_window_t<double>(c, spin * d.n + kk0, cnt) : launch_window_t<float>(c, spin * d.n + kk0, cnt);
+        if (st) return st;
+        st = launch_flush(c, spin);
+        if (st) return st;
+      }
+    bump_sweep_kernel<<<1, 1, 0, c->stream>>>(d.sweep);
+    LAUNCH_CHECK(c);
+    return QMC_OK;
+  }
   {
     ProfScope ps(c, QMC_K_ROW_PROPOSE);
     st = c->is_f64 ? launch_row_propose_t<double>(c, 0, nullptr) : launch_row_propose_t<float>(c, 0, nullptr);
@@ -506,7 +527,8 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
                          (const void*)ratio_grad_kernel<float>, (const void*)ratio_grad_kernel<double>,
                          (const void*)accept_kernel<float>, (const void*)accept_kernel<double>,
                          (const void*)move_fused_kernel<float, true>, (const void*)move_fused_kernel<float, false>,
-                         (const void*)move_fused_kernel<double, true>, (const void*)move_fused_kernel<double, false>};
+                         (const void*)move_fused_kernel<double, true>, (const void*)move_fused_kernel<double, false>,
+                         (const void*)window_kernel<float>, (const void*)window_kernel<double>};
     for (const void* f : fns) {
       e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
       if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
