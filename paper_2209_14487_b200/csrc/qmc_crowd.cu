@@ -16,6 +16,7 @@
 #include "move.cuh"
 #include "spline.cuh"
 #include "update.cuh"
+#include "window.cuh"
 
 using namespace qmc;
 
@@ -312,19 +313,19 @@ int launch_flush(qmc_crowd* c, int spin)
   const size_t flush_smem = 0;
   switch (d.kdp) {
     case 8:
-      flush_finalize_kernel<8><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_finalize_kernel<8><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<1><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     case 16:
-      flush_finalize_kernel<16><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_finalize_kernel<16><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<2><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     case 32:
-      flush_finalize_kernel<32><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_finalize_kernel<32><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<4><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     case 64:
-      flush_finalize_kernel<64><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d);
+      flush_finalize_kernel<64><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<8><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     default: return fail(QMC_ERR_INVALID_ARG, "unsupported padded delay rank %d", d.kdp);
@@ -359,22 +360,22 @@ int step_accept(qmc_crowd* c, int k, unsigned char* acc)
   return c->is_f64 ? launch_accept_t<double>(c, k, acc) : launch_accept_t<float>(c, k, acc);
 }
 
-// one full sweep, D:C6 flush schedule; no host synchronisation (capturable)
 template <typename T>
-int launch_fused_t(qmc_crowd* c, int k, bool next)
+int launch_ratio_accept_t(qmc_crowd* c, int k)
 {
-  ProfScope ps(c, next ? QMC_K_FUSED_MOVE : QMC_K_RATIO_ACCEPT);
-  if (next) move_fused_kernel<T, true><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k);
-  else move_fused_kernel<T, false><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k);
+  ProfScope ps(c, QMC_K_RATIO_ACCEPT);
+  ratio_accept_kernel<T><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
+
+size_t window_smem(const CrowdDev& d, size_t elem) { return (size_t)win_layout(d.N, d.ns, d.kdp, (int)elem).total * 8; }
 
 template <typename T>
 int launch_window_t(qmc_crowd* c, int k0, int cnt)
 {
   ProfScope ps(c, QMC_K_WINDOW);
-  window_kernel<T><<<c->dev.W, MOVE_NT, move_smem(c->dev), c->stream>>>(c->dev, k0, cnt);
+  window_kernel<T><<<c->dev.W, MOVE_NT, window_smem(c->dev, sizeof(T)), c->stream>>>(c->dev, k0, cnt);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
@@ -411,22 +412,14 @@ int sweep_once(qmc_crowd* c)
       st = c->is_f64 ? launch_spline_t<double>(c) : launch_spline_t<float>(c);
     }
     if (st) return st;
-    const int kk = k % d.n;
-    const bool flush_due = d.kd > 1 && (((kk + 1) % d.kd) == 0 || kk == d.n - 1);
-    const bool last = k == d.N - 1;
-    const bool fuse_next = d.kd > 1 && !flush_due && !last;
-    st = c->is_f64 ? launch_fused_t<double>(c, k, fuse_next) : launch_fused_t<float>(c, k, fuse_next);
+    st = c->is_f64 ? launch_ratio_accept_t<double>(c, k) : launch_ratio_accept_t<float>(c, k);
     if (st) return st;
-    if (d.kd == 1) {
+    {
       ProfScope ps(c, QMC_K_RANK1);
       st = c->is_f64 ? launch_rank1_t<double>(c, k) : launch_rank1_t<float>(c, k);
       if (st) return st;
     }
-    if (flush_due) {
-      st = launch_flush(c, k / d.n);
-      if (st) return st;
-    }
-    if (!fuse_next && !last) {
+    if (k + 1 < d.N) {
       ProfScope ps(c, QMC_K_ROW_PROPOSE);
       st = c->is_f64 ? launch_row_propose_t<double>(c, k + 1, nullptr) : launch_row_propose_t<float>(c, k + 1, nullptr);
       if (st) return st;
@@ -521,16 +514,22 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   e = cudaMemcpyAsync(d.R, pos_dev, (size_t)d.W * d.N * 3 * 8, cudaMemcpyDeviceToDevice, c->stream);
   if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "position copy: %s", cudaGetErrorString(e)));
   c->launches += 2;
-  if (move_smem(d) > 48 * 1024) {
-    const int sm = (int)move_smem(d);
+  {
+    const int sm = (int)move_smem(d), wsm = (int)window_smem(d, c->elem);
+    if (wsm > 227 * 1024 || sm > 227 * 1024)
+      return bail(fail(QMC_ERR_INVALID_ARG, "n_elec / delay_rank too large: the per-walker state (%d bytes) exceeds shared memory", wsm));
     const void* fns[] = {(const void*)row_propose_kernel<float>, (const void*)row_propose_kernel<double>,
                          (const void*)ratio_grad_kernel<float>, (const void*)ratio_grad_kernel<double>,
                          (const void*)accept_kernel<float>, (const void*)accept_kernel<double>,
-                         (const void*)move_fused_kernel<float, true>, (const void*)move_fused_kernel<float, false>,
-                         (const void*)move_fused_kernel<double, true>, (const void*)move_fused_kernel<double, false>,
-                         (const void*)window_kernel<float>, (const void*)window_kernel<double>};
+                         (const void*)ratio_accept_kernel<float>, (const void*)ratio_accept_kernel<double>};
     for (const void* f : fns) {
+      if (sm <= 48 * 1024) break;
       e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+      if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
+    }
+    if (wsm > 48 * 1024) {
+      e = c->is_f64 ? cudaFuncSetAttribute(window_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm)
+                    : cudaFuncSetAttribute(window_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm);
       if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
     }
   }

@@ -113,14 +113,15 @@ __device__ __forceinline__ void ld32(const double* p, double (&v)[4])
   v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
 }
 
-// Flush, step 1 (per walker, column-local, in place): C <- Z = S^-T C, Z[l][j] = sum_q Sinv[q][l] C[q][j],
-// so that the strip kernel needs two GEMMs only: B <- B0 - (B0 V^T - E) Z.  A thread owns one column j
-// and up to 32 output rows l in registers, streams C[q][j] once, and reads Sinv from shared memory
-// as warp-wide broadcasts; all reads of a column finish (barrier) before it is overwritten.
+// Flush, step 1 (per walker, column-local): Z = S^-T C, Z[l][j] = sum_q Sinv[q][l] C[q][j], written to
+// the d.C buffer, so that the strip kernel needs two GEMMs only: B <- B0 - (B0 V^T - E) Z.  C[q] is read
+// where it lives, C[q,:] = B0[rows[q],:] (the window kernel never copies it; the strip kernel has not
+// touched B0 yet).  A thread owns one column j and up to 32 output rows l in registers, streams
+// C[q][j] once, and reads Sinv from shared memory as warp-wide broadcasts.
 // 2 k^2 n flop per walker (4 % of the flush at k = 32, n = 384), done once instead of once per strip.
 // grid = (ceil(ns / (FINALIZE_NT / LH)), W), LH = KDP / min(KDP, 32); dynamic smem: KDP*KDP doubles
 template <int KDP>
-__global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d)
+__global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d, int spin)
 {
   constexpr int ZL = KDP < 32 ? KDP : 32;
   constexpr int LH = KDP / ZL;
@@ -131,19 +132,22 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d)
   if (m == 0) return;
   const int ns = d.ns;
   const double* Sinv = d.Sinv + (size_t)w * KDP * KDP;
-  for (int e = threadIdx.x; e < KDP * KDP; e += FINALIZE_NT) s_sinv[e] = Sinv[e];
+  __shared__ int s_rows[KDP];
+  for (int e = threadIdx.x; e < KDP * KDP; e += FINALIZE_NT) s_sinv[e] = (e / KDP < m && e % KDP < m) ? Sinv[e] : 0.0;
+  for (int e = threadIdx.x; e < KDP; e += FINALIZE_NT) s_rows[e] = e < m ? d.rows[(size_t)w * KDP + e] : 0;
   __syncthreads();
   const int half = threadIdx.x / COLS;
   const int j = blockIdx.x * COLS + (threadIdx.x - half * COLS);
   const int l0 = half * ZL;
   double* C = d.C + (size_t)w * KDP * ns + j;
+  const double* B0 = d.Binv + ((size_t)w * 2 + spin) * ns * ns + j;
   double z[ZL];
 #pragma unroll
   for (int l = 0; l < ZL; ++l) z[l] = 0.0;
   if (j < ns && l0 < m) {
 #pragma unroll 2
     for (int q = 0; q < m; ++q) {
-      const double c = C[(size_t)q * ns];
+      const double c = B0[(size_t)s_rows[q] * ns];
 #pragma unroll
       for (int l = 0; l < ZL; ++l) z[l] = fma(s_sinv[q * KDP + l0 + l], c, z[l]);
     }
