@@ -8,7 +8,8 @@
 //                                  position (D:A12, A13); T = table type
 //   vgl    T    [W][5][ns]         phi, d/dx, d/dy, d/dz, lap at the proposed position
 //   brow   fp64 [W][ns]            inverse row of the moved electron, window applied (D:C6)
-//   V, C   fp64 [W][kdp][ns]       delayed window rows; kdp = delay rank padded to 8/16/32/64
+//   V, C, Cp fp64 [W][kdp][ns]     delayed window rows (C doubles as Bcur / Z, Cp = c_l of the window
+//                                  kernel); kdp = delay rank padded to 8/16/32/64
 //   Sinv   fp64 [W][kdp][kdp]      inverse of S = V C^T, grown by bordering
 //   per-walker scalars of the move in flight (rnew, delta, g_old, g_new, ...)
 #pragma once
@@ -36,7 +37,7 @@ struct CrowdDev {
   double *rnew, *delta, *g_old, *g_new;      // [W][3]
   double *usum_old, *rho_d, *rho_j, *p, *u;  // [W]
   unsigned char* accepted;                   // [W]
-  double *V, *C, *Sinv, *pvec, *yvec;
+  double *V, *C, *Cp, *Sinv, *pvec, *yvec;
   int* rows;                                 // [W][kdp]
   int* mwin;                                 // [W]
   unsigned long long* counters;              // [0] accepted moves

@@ -138,15 +138,32 @@ __device__ __forceinline__ void sinv_matvec(const double* Sinv, int ss, int m, c
   }
 }
 
+// Piece 0..4 of the Box-Muller Gaussians of move (walker w, electron k, current sweep) (D:C7):
+// chi = (g0 g1, g0 g2, g3 g4), g0 = sqrt(-2 ln u0), g1 = cos 2 pi u1, g2 = sin 2 pi u1, g3 = sqrt(-2 ln u2),
+// g4 = cos 2 pi u3.  One thread per piece; the pieces depend on nothing but the counter, so the window
+// kernel computes them ahead of time, off the critical path.
+__device__ __forceinline__ double gauss_piece(const CrowdDev& d, int w, int k, int piece)
+{
+  unsigned x[4];
+  philox4x32_10((unsigned)(d.walker_id0 + w), (unsigned)k, *d.sweep, 0u, d.seed_lo, d.seed_hi, x);
+  const double two_pi = 6.283185307179586476925286766559;
+  if (piece == 0) return sqrt(-2.0 * log(u01(x[0])));
+  if (piece == 1) return cos(two_pi * u01(x[1]));
+  if (piece == 2) return sin(two_pi * u01(x[1]));
+  if (piece == 3) return sqrt(-2.0 * log(u01(x[2])));
+  return cos(two_pi * u01(x[3]));
+}
+
 // ---- G_k(R) and the proposal (qmc_spo_vgl step (b)) -------------------------------------------
 // G_k(R) = b . grad phi(r_k) [cache] + grad_k ln Psi_J(R)                       (D:C2, C3, A13)
 // Delta = fl32(tau G + sqrt(tau) chi), r' = r_k + Delta, chi by Box-Muller      (D:C4, C7)
 // b_s: the inverse row of electron k with the window applied (shared memory); cache: [4][ns] of
 // electron k; R: positions [N][3] of the walker.  The five transcendental pieces of the Gaussians
-// run on five threads.  Results go to ms (thread 0); callers synchronise before reading them.
+// run on five threads (or arrive precomputed in gauss_pre[5]).  Results go to ms (thread 0); callers synchronise before reading them.
 template <typename T>
 __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k, const double* b_s, const T* cache,
-                                                 const double* R, const double* rnew_given, MoveScal ms, double* red)
+                                                 const double* R, const double* rnew_given, MoveScal ms, double* red,
+                                                 const double* gauss_pre = nullptr)
 {
   const int ns = d.ns, tid = threadIdx.x;
   // v[0..2] = b . grad phi(r_k), v[3] = usum_old, v[4..6] = grad_k ln Psi_J(R)
@@ -164,21 +181,11 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
     v[4] = g[0]; v[5] = g[1]; v[6] = g[2];
   }
   block_sum<7, MOVE_NT>(v, red);
-  if (!rnew_given) {
-    if (tid < 5) {
-      unsigned x[4];
-      philox4x32_10((unsigned)(d.walker_id0 + w), (unsigned)k, *d.sweep, 0u, d.seed_lo, d.seed_hi, x);
-      const double two_pi = 6.283185307179586476925286766559;
-      double r;
-      if (tid == 0) r = sqrt(-2.0 * log(u01(x[0])));
-      else if (tid == 1) r = cos(two_pi * u01(x[1]));
-      else if (tid == 2) r = sin(two_pi * u01(x[1]));
-      else if (tid == 3) r = sqrt(-2.0 * log(u01(x[2])));
-      else r = cos(two_pi * u01(x[3]));
-      red[tid] = r;
-    }
+  if (!rnew_given && !gauss_pre) {
+    if (tid < 5) red[tid] = gauss_piece(d, w, k, tid);
     __syncthreads();
   }
+  const double* gp = gauss_pre ? gauss_pre : red;
   if (tid == 0) {
     const double g_old[3] = {v[0] + v[4], v[1] + v[5], v[2] + v[6]};
     double delta[3], rn[3];
@@ -186,7 +193,7 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
 #pragma unroll
       for (int c = 0; c < 3; ++c) { rn[c] = rnew_given[3 * (size_t)w + c]; delta[c] = rn[c] - rk[c]; }
     } else {
-      const double chi[3] = {red[0] * red[1], red[0] * red[2], red[3] * red[4]};
+      const double chi[3] = {gp[0] * gp[1], gp[0] * gp[2], gp[3] * gp[4]};
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         const double xx = __dadd_rn(__dmul_rn(d.tau, g_old[c]), __dmul_rn(d.sqrt_tau, chi[c]));

@@ -142,6 +142,7 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
   char* acc_sink = take(W);
   char* V = take(ds->delay_rank > 1 ? W * kdp * ns * 8 : 8);
   char* C = take(ds->delay_rank > 1 ? W * kdp * ns * 8 : 8);
+  char* Cp = take(ds->delay_rank > 1 ? W * kdp * ns * 8 : 8);
   char* Sinv = take(ds->delay_rank > 1 ? W * kdp * kdp * 8 : 8);
   char* pvec = take(W * kdp * 8);
   char* yvec = take(W * kdp * 8);
@@ -155,7 +156,7 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
     d->rnew = (double*)rnew; d->delta = (double*)delta; d->g_old = (double*)g_old; d->g_new = (double*)g_new;
     d->usum_old = (double*)usum_old; d->rho_d = (double*)rho_d; d->rho_j = (double*)rho_j;
     d->p = (double*)p; d->u = (double*)u; d->accepted = (unsigned char*)accepted;
-    d->V = (double*)V; d->C = (double*)C; d->Sinv = (double*)Sinv; d->pvec = (double*)pvec; d->yvec = (double*)yvec;
+    d->V = (double*)V; d->C = (double*)C; d->Cp = (double*)Cp; d->Sinv = (double*)Sinv; d->pvec = (double*)pvec; d->yvec = (double*)yvec;
     d->rows = (int*)rows; d->mwin = (int*)mwin; d->counters = (unsigned long long*)counters;
     d->sweep = (unsigned*)sweep; d->status = (int*)status;
     (void)acc_sink;
@@ -301,7 +302,7 @@ int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
   return QMC_OK;
 }
 
-int launch_flush(qmc_crowd* c, int spin)
+int launch_flush(qmc_crowd* c, int spin, bool from_window = false)
 {
   const CrowdDev& d = c->dev;
   const int rows_per_cta = (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP;
@@ -309,23 +310,27 @@ int launch_flush(qmc_crowd* c, int spin)
   ProfScope ps(c, QMC_K_FLUSH);
   const int fcols = FINALIZE_NT / (d.kdp > 32 ? d.kdp / 32 : 1);
   dim3 fgrid((d.ns + fcols - 1) / fcols, d.W);
-  const size_t fsm = (size_t)d.kdp * d.kdp * 8;
+  const size_t fsm = (size_t)d.kdp * d.kdp * 8, tsm = (size_t)d.kdp * (d.kdp + 1) * 8;
   const size_t flush_smem = 0;
   switch (d.kdp) {
     case 8:
-      flush_finalize_kernel<8><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
+      if (from_window) flush_finalize_tri_kernel<8><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
+      else flush_finalize_kernel<8><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<1><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     case 16:
-      flush_finalize_kernel<16><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
+      if (from_window) flush_finalize_tri_kernel<16><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
+      else flush_finalize_kernel<16><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<2><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     case 32:
-      flush_finalize_kernel<32><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
+      if (from_window) flush_finalize_tri_kernel<32><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
+      else flush_finalize_kernel<32><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<4><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     case 64:
-      flush_finalize_kernel<64><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
+      if (from_window) flush_finalize_tri_kernel<64><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
+      else flush_finalize_kernel<64><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
       flush_kernel<8><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
       break;
     default: return fail(QMC_ERR_INVALID_ARG, "unsupported padded delay rank %d", d.kdp);
@@ -394,7 +399,7 @@ int sweep_once(qmc_crowd* c)
         const int cnt = d.n - kk0 < d.kd ? d.n - kk0 : d.kd;
         st = c->is_f64 ? launch_window_t<double>(c, spin * d.n + kk0, cnt) : launch_window_t<float>(c, spin * d.n + kk0, cnt);
         if (st) return st;
-        st = launch_flush(c, spin);
+        st = launch_flush(c, spin, true);
         if (st) return st;
       }
     bump_sweep_kernel<<<1, 1, 0, c->stream>>>(d.sweep);

@@ -116,13 +116,17 @@ __device__ __forceinline__ double shfl_xor_t(double v, int m) { return __shfl_xo
 // All orbitals at position r by the whole CTA (NT threads, NT % 32 == 0).  `s` is shared memory;
 // `vgl` (global or shared) receives [5][ns]: phi, d/dx, d/dy, d/dz, laplacian, zero beyond M.
 // Contains two __syncthreads(); must be called by all threads of the CTA.
-template <typename T, int NT>
-__device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, SplineW<T>& s, T* vgl)
+// `side(tid)` runs on the threads of warps >= 1 while three threads of warp 0 build the weights
+// (a slot for work that is off the caller's critical path).
+struct NoSideWork { __device__ __forceinline__ void operator()(int) const {} };
+template <typename T, int NT, typename Side = NoSideWork>
+__device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, SplineW<T>& s, T* vgl, Side side = Side())
 {
   constexpr int VW = Vec16<T>::W;
   const int tid = threadIdx.x, a = tid & 3, g = tid >> 2;
   __syncthreads();  // previous users of `s` are done
   if (tid < 3) spline_axis<T>(d, tid, r[tid], s);
+  else if (tid >= 32) side(tid);
   __syncthreads();
   const T* tab = static_cast<const T*>(d.coefs);
   const unsigned chunks = (unsigned)d.ns / VW;

@@ -160,6 +160,78 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d,
   }
 }
 
+// Flush, step 1 for the window kernel's eager-block form (window.cuh, R5): the accepted moves
+// left V[l] = phi_l and Cp[l] = c_l = b_l / rho_l; with N[j][l] = c_j . phi_l (j < l, strictly upper
+// triangular) the Sherman-Morrison chain B_m = B0 - sum_l w_l c_l^T, w_l = B_l phi_l - e_l, telescopes to
+// B_m = B0 - (B0 V^T - E) Z with (I + N) Z = Cp.  One CTA per walker: N by DMMA tiles (operand
+// fragments straight from the rows of Cp and V, as in the strip kernel), then back substitution, one
+// column per thread, Z written to the d.C buffer.  m^2 n + m^2 n / 2 flop per walker (5 % of the flush).
+// grid = W; dynamic smem: KDP*(KDP+1) doubles
+constexpr int FINTRI_NT = 128;
+template <int KDP>
+__global__ void __launch_bounds__(FINTRI_NT) flush_finalize_tri_kernel(CrowdDev d)
+{
+  constexpr int KB = KDP / 8, SS = KDP + 1;
+  extern __shared__ double s_n[];
+  const int w = blockIdx.x;
+  const int m = d.mwin[w];
+  if (m == 0) return;
+  const int ns = d.ns, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+  const double* Cp = d.Cp + (size_t)w * KDP * ns;
+  const double* V = d.V + (size_t)w * KDP * ns;
+  double* Z = d.C + (size_t)w * KDP * ns;
+  for (int e = tid; e < KDP * SS; e += FINTRI_NT) s_n[e] = 0.0;
+  __syncthreads();
+  for (int jb = warp; jb < KB && 8 * jb < m; jb += FINTRI_NT / 32) {
+    double acc[KB][2];
+#pragma unroll
+    for (int lb = 0; lb < KB; ++lb) acc[lb][0] = acc[lb][1] = 0.0;
+    const bool a_ok = 8 * jb + g < m;
+    const double* ap = Cp + (size_t)(8 * jb + g) * ns + 4 * t;
+    const double* vp = V + (size_t)g * ns + 4 * t;
+    for (int s = 0; s < ns; s += 16) {
+      double a[4] = {0.0, 0.0, 0.0, 0.0};
+      if (a_ok) ld32(ap + s, a);
+      double b[KB][4];
+#pragma unroll
+      for (int lb = 0; lb < KB; ++lb) {
+        b[lb][0] = b[lb][1] = b[lb][2] = b[lb][3] = 0.0;
+        if (lb >= jb && 8 * lb + g < m) ld32(vp + (size_t)(8 * lb) * ns + s, b[lb]);
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+#pragma unroll
+        for (int lb = 0; lb < KB; ++lb)
+          if (lb >= jb) dmma884(acc[lb], a[q], b[lb][q]);
+    }
+#pragma unroll
+    for (int lb = 0; lb < KB; ++lb)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int j = 8 * jb + g, l = 8 * lb + 2 * t + e;
+        if (lb >= jb && j < l && l < m) s_n[j * SS + l] = acc[lb][e];
+      }
+  }
+  __syncthreads();
+  for (int col = tid; col < ns; col += FINTRI_NT) {
+    double z[KDP];
+#pragma unroll
+    for (int l = 0; l < KDP; ++l) z[l] = (l < m) ? Cp[(size_t)l * ns + col] : 0.0;
+#pragma unroll
+    for (int l = KDP - 2; l >= 0; --l) {
+      if (l < m - 1) {
+        double a = z[l];
+#pragma unroll
+        for (int j = l + 1; j < KDP; ++j) a = fma(-s_n[l * SS + j], z[j], a);
+        z[l] = a;
+      }
+    }
+#pragma unroll
+    for (int l = 0; l < KDP; ++l)
+      if (l < m) Z[(size_t)l * ns + col] = z[l];
+  }
+}
+
 // ---- strip kernel: fragments straight from global memory, software-pipelined in registers -------
 // (A shared-memory cp.async ring for the operands was measured slower on B200: 2.54 ms vs 2.07 ms per
 // flush at cfg 5 / W = 2048 -- the LDS + LDGSTS instruction stream saturates the MIO queue next to

@@ -1,24 +1,26 @@
 // window.cuh -- qmc_sweep with a delayed update: one launch per delay window, one CTA per walker.
 //
 // The crowd advances in lock-step per *window* (D:C6 schedule): a CTA owns one walker for the
-// cnt <= delay_rank consecutive moves k0 .. k0+cnt-1 (row/proposal, spline, ratio, decision, append
+// cnt <= delay_rank consecutive moves k0 .. k0+cnt-1 (row/proposal, spline, ratio, decision, update
 // for each), then the whole crowd flushes (update.cuh).  Walkers never interact inside a window, so
 // no kernel boundary is needed between moves: an SM overlaps the DRAM-bound spline gather of one
 // walker with the fp64 work of its other resident walkers, the per-walker state (positions, inverse
-// row, orbitals at r', S^-1, the table T) lives in shared memory for the whole window, and the launch
-// tail is paid once per window instead of twice per move.
+// row, orbitals at r') lives in shared memory for the whole window, and the launch tail is paid once
+// per window instead of twice per move.
 //
-// Because the electrons of a window are consecutive, the rows B0[k0 .. k0+cnt) the window will ever
-// need (as proposal rows and, once accepted, as rows of C) form one contiguous block `blk` of the
-// transposed inverse that nobody writes before the flush.  On an accepted move l (orbital vector
-// V[l] = phi') the kernel takes ONE pass over that block, T[l][i] = blk[i] . V[l], which yields
-//   - p_l = V[l] . B0[k] for every later move k = k0 + i of the window     (column i of T),
-//   - q_j = C[j] . phi' = blk[i_j] . V[l] for the earlier accepted rows     (entries T[l][i_j]),
-//   - the corner B0[k] . phi'                                                (entry T[l][i]).
-// So V is only written (for the flush GEMM), C is never materialised (C[l] = blk[i_l]), and a move
-// reads the block twice (axpy for the row, T pass on accept) instead of V + C + C.
-// The dots use the same lane/shuffle summation trees as the step kernels (move.cuh), so qmc_sweep and
-// the three step calls give bit-identical trajectories.
+// Inside the window the kernel uses the *eager-block* form of the delayed update (R5).
+// Because the electrons of a window are consecutive, the only inverse rows the window itself needs
+// are the cnt rows `blk` = B0[k0 .. k0+cnt); every accepted move l (row k_l, orbitals phi_l, ratio
+// rho_l, current row b_l) applies its Sherman-Morrison update (D:C5) to the rows of that block that
+// are still to be proposed,
+//     Bcur[i'] <- Bcur[i'] - (Bcur[i'] . phi_l) c_l,     c_l = b_l / rho_l,      i' after the move,
+// so that the row of the next move is simply Bcur[i] -- no S^-1, no p/q vectors, no axpy over the
+// window -- and one pass over (on average) half the block per accepted move is all the window traffic.
+// The other n - cnt rows get the same updates at the flush: with V[l] = phi_l, Cp[l] = c_l and the
+// strictly upper triangular N[j][l] = c_j . phi_l (j < l),
+//     B <- B0 - (B0 V^T - E) Z,      (I + N) Z = Cp,
+// which is C6's B0 - (B0 V^T - E) S^-T C with the bordered inverse replaced by its unit-triangular
+// factor (flush_finalize_tri_kernel); the two-GEMM strip kernel is the same for both paths.
 #pragma once
 #include "move.cuh"
 
@@ -30,26 +32,22 @@ namespace qmc {
 
 // Shared-memory layout of the window kernel, offsets in doubles.
 struct WinLayout {
-  int R, b, Sinv, Tm, p, y, q, z, red, mv, misc, rows, vgl, total;
+  int R, b, bn, red, mv, gauss, rows, cbuf, vgl, total;
 };
 __host__ __device__ inline WinLayout win_layout(int N, int ns, int kdp, int elem)
 {
   WinLayout L;
   int o = 0;
-  L.R = o; o += 3 * N;               // positions of the walker
-  L.b = o; o += ns;                  // inverse row of the move, window applied
-  L.Sinv = o; o += kdp * (kdp + 1);  // S^-1, row stride kdp + 1 (bank spread)
-  L.Tm = o; o += kdp * kdp;          // T[l][i] = blk[i] . V[l]
-  L.p = o; o += kdp;
-  L.y = o; o += kdp;
-  L.q = o; o += kdp;
-  L.z = o; o += kdp;
+  L.R = o; o += 3 * N;       // positions of the walker
+  L.b = o; o += ns;          // inverse row of the current move (then c_l = b / rho_D)
+  L.bn = o; o += ns;         // inverse row of the next move
   L.red = o; o += MOVE_RED;
   L.mv = o; o += MOVE_MV;
-  L.misc = o; o += 16;
-  L.rows = o; o += kdp / 2;          // int[kdp]: window-local index of accepted move l
+  L.gauss = o; o += 8;       // Box-Muller pieces of the next move
+  L.rows = o; o += kdp / 2;  // int[kdp]: electron (within the spin block) of accepted move l
   o = (o + 1) & ~1;
-  L.vgl = o; o += (5 * ns * elem + 7) / 8;  // orbitals at r': T[5][ns]
+  L.cbuf = o; o += 2 * ((3 * ns * elem + 15) / 16) * 2;  // gradient cache of this / the next move: 2 x T[3][ns]
+  L.vgl = o; o += (5 * ns * elem + 7) / 8;               // orbitals at r': T[5][ns]
   L.total = o;
   return L;
 }
@@ -61,102 +59,179 @@ __device__ __forceinline__ double2 ld_x2(const float* v, int jj)
 }
 __device__ __forceinline__ double2 ld_x2(const double* v, int jj) { return reinterpret_cast<const double2*>(v)[jj]; }
 
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// 16-byte asynchronous copy global -> shared through L2 only (the sources are lines this CTA or the flush
+// wrote earlier; L1 is not involved).  SASS: LDGSTS.
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
+{
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// nbytes % 16 == 0, both 16-byte aligned; strided over the CTA
+__device__ __forceinline__ void cp_async_cta(void* smem, const void* gmem, int nbytes)
+{
+  for (int o = threadIdx.x * 16; o < nbytes; o += MOVE_NT * 16)
+    cp_async16(static_cast<char*>(smem) + o, static_cast<const char*>(gmem) + o);
+}
+
+// Sherman-Morrison on the rows of the window block that are still to be proposed (D:C5 restricted to the
+// block): for rows r in [r_first, cnt): t = src[r] . phi', dst[r] = src[r] - t c, with phi' = vgl_s[0..ns)
+// and c = c_s (both shared memory).  A warp takes two rows at a time, keeps them in registers between the
+// dot and the update (rows of up to 64 WIN_NV = 512 columns; longer rows are read twice), and also
+// hands row r_first to shared memory (next_s) as the next move's inverse row.
+constexpr int WIN_NV = 8;
+template <typename T>
+__device__ __forceinline__ void block_rows_update(const double* src, double* dst, int ns, int r_first, int cnt,
+                                                  const T* vgl_s, const double* c_s, double* next_s)
+{
+  constexpr int RB = 2;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nh = ns / 2;
+  const double2* c2 = reinterpret_cast<const double2*>(c_s);
+  if (nh <= 32 * WIN_NV) {
+    for (int r0 = r_first + warp * RB; r0 < cnt; r0 += MOVE_NW * RB) {
+      double2 v[RB][WIN_NV];
+      double acc[RB];
+#pragma unroll
+      for (int r = 0; r < RB; ++r) {
+        acc[r] = 0.0;
+        const double2* rp = reinterpret_cast<const double2*>(src + (size_t)(r0 + r) * ns);
+#pragma unroll
+        for (int q = 0; q < WIN_NV; ++q) {
+          const int jj = lane + 32 * q;
+          v[r][q] = (r0 + r < cnt && jj < nh) ? rp[jj] : make_double2(0.0, 0.0);
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < WIN_NV; ++q) {
+        const int jj = lane + 32 * q;
+        if (jj < nh) {
+          const double2 x = ld_x2(vgl_s, jj);
+#pragma unroll
+          for (int r = 0; r < RB; ++r) acc[r] = fma(v[r][q].x, x.x, fma(v[r][q].y, x.y, acc[r]));
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < RB; ++r) acc[r] = warp_sum(acc[r]);
+#pragma unroll
+      for (int r = 0; r < RB; ++r) {
+        if (r0 + r < cnt) {
+          double2* wp = reinterpret_cast<double2*>(dst + (size_t)(r0 + r) * ns);
+          double2* sp = (r0 + r == r_first) ? reinterpret_cast<double2*>(next_s) : nullptr;
+#pragma unroll
+          for (int q = 0; q < WIN_NV; ++q) {
+            const int jj = lane + 32 * q;
+            if (jj < nh) {
+              const double2 c = c2[jj];
+              const double2 o = make_double2(fma(-acc[r], c.x, v[r][q].x), fma(-acc[r], c.y, v[r][q].y));
+              wp[jj] = o;
+              if (sp) sp[jj] = o;
+            }
+          }
+        }
+      }
+    }
+  } else {
+    for (int r = r_first + warp; r < cnt; r += MOVE_NW) {
+      const double2* rp = reinterpret_cast<const double2*>(src + (size_t)r * ns);
+      double2* wp = reinterpret_cast<double2*>(dst + (size_t)r * ns);
+      double acc = 0.0;
+      for (int jj = lane; jj < nh; jj += 32) {
+        const double2 x = ld_x2(vgl_s, jj), v = rp[jj];
+        acc = fma(v.x, x.x, fma(v.y, x.y, acc));
+      }
+      acc = warp_sum(acc);
+      for (int jj = lane; jj < nh; jj += 32) {
+        const double2 c = c2[jj], v = rp[jj];
+        const double2 o = make_double2(fma(-acc, c.x, v.x), fma(-acc, c.y, v.y));
+        wp[jj] = o;
+        if (r == r_first) reinterpret_cast<double2*>(next_s)[jj] = o;
+      }
+    }
+  }
+}
 
 // dynamic smem: win_layout(...).total doubles.  Requires an empty window on entry (qmc_sweep flushes first).
+// Leaves for the flush: V[l] = phi_l, Cp[l] = c_l, rows[l], mwin (and Bcur in the d.C buffer, dead afterwards).
 template <typename T>
 __global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(CrowdDev d, int k0, int cnt)
 {
   extern __shared__ double sm[];
   __shared__ SplineW<T> sw;
-  const int w = blockIdx.x, ns = d.ns, kdp = d.kdp, ss = kdp + 1, tid = threadIdx.x;
+  const int w = blockIdx.x, ns = d.ns, kdp = d.kdp, tid = threadIdx.x;
   const WinLayout L = win_layout(d.N, ns, kdp, (int)sizeof(T));
   double* R_s = sm + L.R;
-  double* b_s = sm + L.b;
-  double* Sinv_s = sm + L.Sinv;
-  double* T_s = sm + L.Tm;
-  double* p_s = sm + L.p;
-  double* y_s = sm + L.y;
-  double* q_s = sm + L.q;
-  double* z_s = sm + L.z;
+  double* b_s = sm + L.b;    // row of the current move
+  double* bn_s = sm + L.bn;  // row of the next move
   double* red = sm + L.red;
-  double* misc = sm + L.misc;
+  double* gauss = sm + L.gauss;
   int* rows_s = reinterpret_cast<int*>(sm + L.rows);
+  const int cstride = ((3 * ns * (int)sizeof(T) + 15) / 16) * 16 / (int)sizeof(T);
+  T* cbuf = reinterpret_cast<T*>(sm + L.cbuf);
   T* vgl_s = reinterpret_cast<T*>(sm + L.vgl);
   const MoveScal ms = move_scal_smem(sm + L.mv);
 
   const int spin = k0 / d.n, kk0 = k0 - spin * d.n;
-  const double* blk = d.Binv + (((size_t)w * 2 + spin) * ns + kk0) * ns;
+  const double* blk = d.Binv + (((size_t)w * 2 + spin) * ns + kk0) * ns;  // B0 rows of the window
+  double* Bcur = d.C + (size_t)w * kdp * ns;                              // their current values, once m > 0
+  double* Cp = d.Cp + (size_t)w * kdp * ns;
+  double* V = d.V + (size_t)w * kdp * ns;
   double* Rg = d.R + (size_t)w * d.N * 3;
   T* cache0 = static_cast<T*>(d.cache) + ((size_t)w * d.N + k0) * 4 * ns;
-  double* V = d.V + (size_t)w * kdp * ns;
+  const int row_bytes = ns * 8, cache_bytes = 3 * ns * (int)sizeof(T);
 
-  // prologue: positions to shared memory; pull the block and the first gradient cache into L2
+  // prologue: row and gradient cache of the first move, positions, Gaussians of the first move;
+  // the rest of the block is pulled into L2 (first-touch DRAM lines the first accepted move reads)
+  cp_async_cta(b_s, blk, row_bytes);
+  cp_async_cta(cbuf, cache0, cache_bytes);
   for (int j = tid; j < 3 * d.N; j += MOVE_NT) R_s[j] = Rg[j];
-  {
-    const int lines_blk = cnt * ns * 8 / 128, lines_c = 3 * ns * (int)sizeof(T) / 128;
-    for (int j = tid; j < lines_blk + lines_c; j += MOVE_NT)
-      prefetch_l2(j < lines_blk ? reinterpret_cast<const char*>(blk) + (size_t)j * 128
-                                : reinterpret_cast<const char*>(cache0) + (size_t)(j - lines_blk) * 128);
-  }
-  int m = 0;
-  unsigned long long accmask = 0ull;  // window-local indices accepted so far (uniform across the CTA)
+  if (tid >= 32 && tid < 37) gauss[tid - 32] = gauss_piece(d, w, k0, tid - 32);
+  for (int j = tid; j < (cnt - 1) * row_bytes / 128; j += MOVE_NT)
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
+  cp_async_wait_all();
   __syncthreads();
 
+  int m = 0;
   for (int i = 0; i < cnt; ++i) {
     const int k = k0 + i;
-    T* cache = cache0 + (size_t)i * 4 * ns;
-    if (i + 1 < cnt) {  // next move's gradient cache: first-touch DRAM lines
-      const int lines_c = 3 * ns * (int)sizeof(T) / 128;
-      for (int j = tid; j < lines_c; j += MOVE_NT) prefetch_l2(reinterpret_cast<const char*>(cache + 4 * ns) + (size_t)j * 128);
+    T* ccur = cbuf + (i & 1) * cstride;
+    T* cache_g = cache0 + (size_t)i * 4 * ns;
+    const bool more = i + 1 < cnt;
+    if (more) {  // next move's row (valid unless this move is accepted, which rewrites it) and gradient cache
+      cp_async_cta(bn_s, (m ? Bcur : blk) + (size_t)(i + 1) * ns, row_bytes);
+      cp_async_cta(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
     }
-    // ---- row with the window applied (D:C6) ----
-    for (int j = tid; j < ns; j += MOVE_NT) b_s[j] = blk[(size_t)i * ns + j];
-    if (m > 0) {
-      for (int l = tid; l < m; l += MOVE_NT) p_s[l] = T_s[l * kdp + i];  // electron k is not in the window yet
-      __syncthreads();
-      sinv_matvec(Sinv_s, ss, m, p_s, y_s);
-      __syncthreads();
-      axpy_rows(b_s, ns, m, y_s, [&](int l) { return blk + (size_t)rows_s[l] * ns; });
-    }
-    __syncthreads();
-    // ---- G_k(R), proposal, orbitals at r', ratio, decision ----
-    dev_gold_propose<T>(d, w, k, b_s, cache, R_s, nullptr, ms, red);
-    spline_cta<T, MOVE_NT>(d, ms.rn, sw, vgl_s);
+    // ---- G_k(R), proposal, orbitals at r' (the next move's Gaussians ride along), ratio, decision ----
+    dev_gold_propose<T>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss);
+    spline_cta<T, MOVE_NT>(d, ms.rn, sw, vgl_s, [&](int t) {
+      if (more && t < 37) gauss[t - 32] = gauss_piece(d, w, k + 1, t - 32);
+    });
     __syncthreads();
     dev_ratio_grad<T>(d, w, k, b_s, vgl_s, R_s, ms, nullptr, nullptr, red);
+    cp_async_wait_all();
     if (dev_decide(d, w, k, ms, nullptr)) {
-      for (int j = tid; j < 4 * ns; j += MOVE_NT) cache[j] = vgl_s[ns + j];
+      const double inv_rho = 1.0 / *ms.rho_d;
+      for (int j = tid; j < ns; j += MOVE_NT) {
+        const double c = b_s[j] * inv_rho;
+        b_s[j] = c;
+        Cp[(size_t)m * ns + j] = c;
+        V[(size_t)m * ns + j] = (double)vgl_s[j];
+      }
+      for (int j = tid; j < 4 * ns; j += MOVE_NT) cache_g[j] = vgl_s[ns + j];
       if (tid < 3) {
         const double x = ms.rn[tid];
         R_s[3 * k + tid] = x;
         Rg[3 * k + tid] = x;
       }
-      for (int j = tid; j < ns; j += MOVE_NT) V[(size_t)m * ns + j] = (double)vgl_s[j];
-      // T[m][i'] = blk[i'] . phi' for every row still needed: later moves, this move, accepted rows
-      rows_dot<4>(cnt, ns,
-                  [&](int ip) { return (ip >= i || ((accmask >> ip) & 1ull)) ? blk + (size_t)ip * ns : nullptr; },
-                  [&](int jj) { return ld_x2(vgl_s, jj); },
-                  [&](int ip, double acc) { T_s[m * kdp + ip] = acc; });
+      if (tid == 0) rows_s[m] = kk0 + i;
       __syncthreads();
-      for (int l = tid; l < m; l += MOVE_NT) q_s[l] = T_s[m * kdp + rows_s[l]];
-      if (tid == 0) misc[0] = T_s[m * kdp + i];
-      __syncthreads();
-      sinv_border(Sinv_s, ss, m, q_s, y_s, z_s, misc);
-      if (tid == 0) rows_s[m] = i;
-      accmask |= 1ull << i;
+      block_rows_update<T>(m ? Bcur : blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
       ++m;
     }
     __syncthreads();
+    double* t = b_s; b_s = bn_s; bn_s = t;
   }
 
-  // epilogue: what the flush needs, in the global layout of the step path
-  double* Sinv = d.Sinv + (size_t)w * kdp * kdp;
-  for (int e = tid; e < m * m; e += MOVE_NT) {
-    const int a = e / m, b = e - a * m;
-    Sinv[(size_t)a * kdp + b] = Sinv_s[a * ss + b];
-  }
-  for (int l = tid; l < m; l += MOVE_NT) d.rows[(size_t)w * kdp + l] = kk0 + rows_s[l];
+  for (int l = tid; l < m; l += MOVE_NT) d.rows[(size_t)w * kdp + l] = rows_s[l];
   if (tid == 0) d.mwin[w] = m;
 }
 

@@ -86,8 +86,11 @@ def test_graph_replay_equals_plain_launches_and_crowd_split(kd):
 
 @pytest.mark.parametrize("n_elec,kd", [(48, 8), (40, 16), (24, 1)])
 def test_sweep_equals_the_three_step_calls(n_elec, kd):
-    """qmc_sweep runs fused kernels (ratio + accept + next row in one launch); the step calls run the
-    same device functions one per launch.  Both must give bit-identical trajectories."""
+    """qmc_sweep against the three step calls on the same crowd.  delay_rank = 1: same device functions,
+    bit-identical.  delay_rank > 1: qmc_sweep runs the window kernel in the eager-block form of the delayed
+    update (R5), the step calls the bordered-S^-1 form of C6: the two agree to rounding (1e-13),
+    which the fp32 quantisation of the displacement (A7) turns into identical positions and decisions;
+    the inverses agree to 1e-10."""
     wl = qi.small_workload(n_elec=n_elec, grid=10, box=6.0, coef_dtype="f32", coef_dist="normal", n_walkers=7,
                            tau=0.02, delay_rank=kd, cfg=14)
     a, _, _, _ = make_pair(wl)
@@ -105,7 +108,10 @@ def test_sweep_equals_the_three_step_calls(n_elec, kd):
                 b.qmc_flush_delayed()
         assert np.array_equal(npy(a.positions()), npy(b.positions()))
         for spin in (0, 1):
-            assert np.array_equal(npy(a.inverse(spin)), npy(b.inverse(spin)))
+            if kd == 1:
+                assert np.array_equal(npy(a.inverse(spin)), npy(b.inverse(spin)))
+            else:
+                assert relerr(npy(a.inverse(spin)), npy(b.inverse(spin))) < 1e-10
     assert a.stats() == b.stats()
 
 
