@@ -102,15 +102,28 @@ __global__ void __launch_bounds__(RANK1_NT) rank1_generic_kernel(CrowdDev d, int
   }
 }
 
-constexpr int FLUSH_NT = 128;            // 4 warps
+#ifndef QMC_FLUSH_PFD
+#define QMC_FLUSH_PFD 8
+#endif
+#ifndef QMC_FLUSH_MIN_CTAS
+#define QMC_FLUSH_MIN_CTAS 3
+#endif
+#ifndef QMC_FLUSH_NT
+#define QMC_FLUSH_NT 128
+#endif
+constexpr int FLUSH_NT = QMC_FLUSH_NT;    // one 16-row strip per warp
 constexpr int FLUSH_ROWS_PER_WARP = 16;  // two 8-row MMA blocks
 constexpr int FINALIZE_NT = 128;
 
+// 32-byte vector access (sm_100: ld/st.global.v4.f64 -> LDG.E.256 / STG.E.256): one L1 request per lane
+// instead of two; p must be 32-byte aligned.
 __device__ __forceinline__ void ld32(const double* p, double (&v)[4])
 {
-  const double2 a = *reinterpret_cast<const double2*>(p);
-  const double2 b = *reinterpret_cast<const double2*>(p + 2);
-  v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
+}
+__device__ __forceinline__ void st32(double* p, double a, double b, double c, double d)
+{
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
 }
 
 // Flush, step 1 (per walker, column-local): Z = S^-T C, Z[l][j] = sum_q Sinv[q][l] C[q][j], written to
@@ -248,6 +261,13 @@ __device__ __forceinline__ void load_frag1(Frag1<KB>& f, const double* a0p, cons
 {
   ld32(a0p + s, f.a0);
   ld32(a1p + s, f.a1);
+#if QMC_FLUSH_PFD > 0
+  // the strip of B0 is the DRAM stream of this kernel: pull its lines into L2 QMC_FLUSH_PFD chunks ahead
+  if ((threadIdx.x & 3) == 0 && s + 16 * QMC_FLUSH_PFD < ns) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(a0p + s + 16 * QMC_FLUSH_PFD));
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(a1p + s + 16 * QMC_FLUSH_PFD));
+  }
+#endif
 #pragma unroll
   for (int b = 0; b < KB; ++b) {
     f.v[b][0] = f.v[b][1] = f.v[b][2] = f.v[b][3] = 0.0;
@@ -314,15 +334,13 @@ __device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double
           dmma884(do1, nw[1][b][q], f.z[b][q].y);
         }
       }
-  *reinterpret_cast<double2*>(o0) = make_double2(de0[0] + ee0[0], do0[0] + eo0[0]);
-  *reinterpret_cast<double2*>(o0 + 2) = make_double2(de0[1] + ee0[1], do0[1] + eo0[1]);
-  *reinterpret_cast<double2*>(o1) = make_double2(de1[0] + ee1[0], do1[0] + eo1[0]);
-  *reinterpret_cast<double2*>(o1 + 2) = make_double2(de1[1] + ee1[1], do1[1] + eo1[1]);
+  st32(o0, de0[0] + ee0[0], do0[0] + eo0[0], de0[1] + ee0[1], do0[1] + eo0[1]);
+  st32(o1, de1[0] + ee1[0], do1[0] + eo1[0], de1[1] + ee1[1], do1[1] + eo1[1]);
 }
 
 // Flush, step 2: B_strip <- B0_strip - (B0_strip V^T - E) Z.  KB = kdp / 8. grid = (ceil(ns / 64), W).
 template <int KB>
-__global__ void __launch_bounds__(FLUSH_NT, 2) flush_kernel(CrowdDev d, int spin)
+__global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(CrowdDev d, int spin)
 {
   const int w = blockIdx.y;
   const int m = d.mwin[w];
