@@ -4,7 +4,7 @@
 A "step" is one full sweep of the whole hot path (propose, spline VGL, ratio/grad, accept,
 delayed append, DMMA flush) over one crowd: W x N proposed electron moves (reading A18).
 Workload at N=1: BASELINE.json configs[4] (768 electrons, 80^3 fp32 table, delayed rank 32), the
-largest configuration; it fits one GPU.  Crowd size via --walkers (default 2048).
+largest configuration; it fits one GPU.  Crowd size via --walkers (default 4096, the largest crowd of the config).
 
   python bench.py [--gpus N] [--steps K] [--warmup W]        CUDA path, one JSON line
   python bench.py --impl reference ...                        the oracle on the host cores
@@ -40,21 +40,29 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cfg", type=int, default=5, help="BASELINE.json config index 1..5")
-    ap.add_argument("--walkers", type=int, default=2048, help="crowd size W per GPU")
+    ap.add_argument("--walkers", type=int, default=4096, help="crowd size W per GPU (cfg 5: 64..4096)")
     ap.add_argument("--delay-rank", type=int, default=None)
     ap.add_argument("--crowd-sweep", action="store_true", help="also print moves/s vs crowd size and delay rank")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-probes", action="store_true", help="skip the step-call / rank-1 kernel probes")
     ap.add_argument("--ref-walkers", type=int, default=None, help="walkers of the oracle sample (default = cores)")
     return ap.parse_args()
 
 
 def peaks():
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written) or the profiling guide's fallback.
+    FP64 tensor: no measured entry exists, so it is the measured bf16 GEMM peak x the guide's nominal
+    ratio 45 / 2250 (sustained figure: the flush is timed inside a long step)."""
     p = ROOT / "MEASURED_PEAKS.json"
     if p.exists():
         d = json.loads(p.read_text())
-        return {"hbm_gbs": float(d["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)"}
-    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+        bf16 = float(d.get("bf16_tflops_sustained", d.get("bf16_tflops", 1400.0)))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "fp64_tflops": bf16 * 45.0 / 2250.0,
+                "source": "measured (MEASURED_PEAKS.json)",
+                "fp64_source": "measured sustained bf16 GEMM x nominal 45/2250"}
+    return {"hbm_gbs": 6650.0, "fp64_tflops": 1400.0 * 45.0 / 2250.0, "source": "fallback (B200_PROFILING.md)",
+            "fp64_source": "fallback sustained bf16 1.4 PF x nominal 45/2250"}
 
 
 class ClockSampler:
@@ -158,13 +166,14 @@ def run_reference(args):
 # ----------------------------------------------------------------------------------------------
 # algorithmic work per launch
 # ----------------------------------------------------------------------------------------------
-def algorithmic(wl, W, kd, alpha, el):
+def algorithmic(wl, W, kd, alpha, el, m_move=None):
     """Bytes / flops ONE launch of each kernel class moves for a crowd of W walkers, with
     acceptance fraction alpha (mean window fill at a flush = alpha*kd, mean fill at a move
     = alpha*(kd-1)/2)."""
     n = M = wl.n
     N = wl.n_elec
-    m_move = alpha * (kd - 1) / 2 if kd > 1 else 0.0
+    if m_move is None:
+        m_move = alpha * (kd - 1) / 2 if kd > 1 else 0.0
     m_flush = alpha * kd
     ratio_b = W * (8 * n + 4 * M * el + 24 * N)
     accept_b = alpha * W * (8 * M * el + (8 * n * m_move + 3 * 8 * n + M * el if kd > 1 else 0))
@@ -177,9 +186,12 @@ def algorithmic(wl, W, kd, alpha, el):
         "ratio_accept": {"bytes": ratio_b + accept_b},
         # fused ratio(k) + accept(k) + row(k+1): C rows and positions are needed once, not twice
         "fused_move": {"bytes": ratio_b + accept_b + row_b - alpha * W * 8 * n * m_move - W * 24 * N},
-        # one launch = all kd moves of a delay window: spline + ratio + accept + row per move
-        "window": {"bytes": kd * (W * (64 * M * el + 5 * M * el) + ratio_b + accept_b + row_b
-                                  - alpha * W * 8 * n * m_move - W * 24 * N),
+        # one launch = all kd moves of a delay window in the eager-block form (window.cuh): per move the
+        # spline gather, one inverse row and one gradient-cache row; per accepted move the cache / V / Cp
+        # rows written and the still-to-be-proposed rows of the block read and rewritten ((kd-1)/2 on average);
+        # positions once per window.  Orbitals at r' never leave the SM.
+        "window": {"bytes": W * (kd * (64 * M * el + 8 * n + 3 * M * el)
+                                 + alpha * kd * (4 * M * el + 16 * n + 16 * n * (kd - 1) / 2) + 24 * N),
                    "flops": kd * W * 600 * M},
         "rank1": {"bytes": alpha * W * 16 * n * n, "flops": alpha * W * 4 * n * n},
         "flush": {"bytes": W * 16 * n * n, "flops": W * (4 * n * n * m_flush + 2 * n * m_flush ** 2)},
@@ -214,6 +226,19 @@ def time_sweeps(crowd, steps, warmup, sync_all):
     sync_all()
     s1 = crowd.stats()
     return e0.elapsed_time(e1), s1["proposed"] - s0["proposed"], s1["accepted"] - s0["accepted"], crowd.launch_count() - l0
+
+
+def ncu_traffic(cfg, W, kd):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu captures
+    (profiles/r1_dram_traffic.csv: cfg,walkers,delay_rank,kernel,bytes), for the configuration timed here."""
+    out = {}
+    f = ROOT / "profiles" / "r1_dram_traffic.csv"
+    if f.exists():
+        for ln in f.read_text().splitlines():
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) == 5 and c[0].isdigit() and (int(c[0]), int(c[1]), int(c[2])) == (cfg, W, kd):
+                out[c[3]] = float(c[4])
+    return out
 
 
 def fp64_probe():
@@ -269,6 +294,15 @@ def run_cuda(args):
     crowd.set_option(q.QMC_OPT_PROFILE, 1)
     crowd.qmc_sweep(1)
     prof = crowd.profile()
+    step_prof = {}
+    if not args.no_probes and rank == 0:
+        # the same kernels one call at a time (C-ABI step calls), 8 moves: stand-alone spline / row / ratio / accept
+        for k in range(min(8, kd, wl.n)):
+            crowd.qmc_spo_vgl(k)
+            crowd.qmc_ratio_grad(k)
+            crowd.qmc_accept_reject(k)
+        crowd.qmc_flush_delayed()
+        step_prof = {k2: v for k2, v in crowd.profile().items() if v[1] and k2 != "flush"}
     crowd.set_option(q.QMC_OPT_PROFILE, 0)
     tot_ms = sum(v[0] for v in prof.values()) or 1.0
     alg = algorithmic(wl, W, kd, alpha, el)
@@ -284,10 +318,39 @@ def run_cuda(args):
         if "flops" in alg[name]:
             ent["tflops"] = alg[name]["flops"] / (avg * 1e-3) / 1e12
         kernels[name] = ent
+    for name, (kms, cnt) in step_prof.items():
+        if name in kernels or name not in alg:
+            continue
+        avg = kms / cnt
+        a_step = algorithmic(wl, W, kd, alpha, el, m_move=alpha * 3.5)[name]     # window fill 0..7 in the probe
+        ent = {"launches": cnt, "avg_us": 1e3 * avg, "share": 0.0, "gbs": a_step["bytes"] / (avg * 1e-3) / 1e9,
+               "probe": "step calls, 8 moves"}
+        ent["hbm_frac"] = ent["gbs"] / pk["hbm_gbs"]
+        kernels[name] = ent
     dom = max(kernels, key=lambda k: kernels[k]["share"])
+    traffic = ncu_traffic(args.cfg, W, kd)
     roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "frac": kernels[dom]["gbs"] / pk["hbm_gbs"], "traffic": None, "peak_source": pk["source"],
-                "share_of_step": kernels[dom]["share"]}
+                "frac": kernels[dom]["gbs"] / pk["hbm_gbs"], "traffic": traffic.get(dom), "peak_source": pk["source"],
+                "share_of_step": kernels[dom]["share"],
+                "algorithmic_bytes_per_launch": alg[dom]["bytes"]}
+    extra_rooflines = {}
+    if "flush" in kernels:
+        n = wl.n
+        useful = kernels["flush"]["tflops"]
+        kdp = 8
+        while kdp < kd:
+            kdp *= 2
+        executed = useful * (4 * n * n * kdp + 2 * n * kdp * kdp) / max(alg["flush"]["flops"] / W, 1.0)
+        extra_rooflines["flush"] = {
+            "kernel": "flush (finalize + DMMA strip)", "bound": "tensor", "achieved": useful, "peak": pk["fp64_tflops"],
+            "unit": "TFLOP/s", "frac": useful / pk["fp64_tflops"], "traffic": traffic.get("flush"),
+            "peak_source": pk["fp64_source"], "share_of_step": kernels["flush"]["share"],
+            "executed_tflops_with_padding": executed, "hbm_frac": kernels["flush"]["hbm_frac"]}
+    for name in ("spline_vgl", "rank1"):
+        if name in kernels:
+            extra_rooflines[name] = {"kernel": name, "bound": "hbm", "achieved": kernels[name]["gbs"],
+                                     "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": kernels[name]["hbm_frac"],
+                                     "traffic": traffic.get(name), "share_of_step": kernels[name]["share"]}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -298,7 +361,7 @@ def run_cuda(args):
                    "parallelism": f"walkers sharded over {world} GPU(s), no collective",
                    "l2": "working set (table + inverses + caches) is far larger than the 126 MB L2; no flush needed"},
         "accept_fraction": alpha, "gpu_launches": launches, "create_s": create_s,
-        "clocks": clk.summary(), "roofline": roofline, "kernels": kernels,
+        "clocks": clk.summary(), "roofline": roofline, "rooflines": extra_rooflines, "kernels": kernels,
     }
     if rank == 0:
         try:
@@ -326,13 +389,39 @@ def run_cuda(args):
     del crowd
     torch.cuda.empty_cache()
 
+    if rank == 0 and world == 1 and not args.no_probes and kd > 1:
+        # Sherman-Morrison path (delay_rank = 1) on the same crowd size: 16 step moves, rank-1 kernel roofline
+        c1, _ = make_crowd(wl, W, 1, 0, coefs_dev, dev)
+        c1.set_option(q.QMC_OPT_PROFILE, 1)
+        a0 = c1.stats()["accepted"]
+        for k in range(16):
+            c1.qmc_spo_vgl(k)
+            c1.qmc_ratio_grad(k)
+            c1.qmc_accept_reject(k)
+        p1 = c1.profile()
+        a1 = (c1.stats()["accepted"] - a0) / (16.0 * W)
+        kms, cnt = p1["rank1"]
+        if cnt:
+            avg = kms / cnt
+            byts = a1 * W * 16 * wl.n * wl.n
+            ent = {"kernel": "rank1", "bound": "hbm", "achieved": byts / (avg * 1e-3) / 1e9, "peak": pk["hbm_gbs"],
+                   "unit": "GB/s", "traffic": traffic.get("rank1"), "avg_us": 1e3 * avg, "accept_fraction": a1,
+                   "probe": "delay_rank 1 crowd, 16 step moves"}
+            ent["frac"] = ent["achieved"] / pk["hbm_gbs"]
+            line["rooflines"]["rank1"] = ent
+        c1.close()
+        del c1
+        torch.cuda.empty_cache()
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = len(os.sched_getaffinity(0))
-        nw = args.ref_walkers or cores
-        nw *= 2
-        v, threads, dt, a = oracle_sample(wl, kd, nw, 2, coefs_np)
+        nw = (args.ref_walkers or cores) * 2
+        # size the sample for roughly 15 s of CPU work: one timed sweep first, then as many as fit
+        v1, threads, dt1, _ = oracle_sample(wl, kd, nw, 1, coefs_np)
+        n_sw = int(min(max(round(15.0 / max(dt1, 1e-3)), 2), 40))
+        v, threads, dt, a = oracle_sample(wl, kd, nw, n_sw, coefs_np)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                "sample": f"{nw} walkers x 2 sweeps of the same workload ({dt:.1f} s wall)",
+                                "sample": f"{nw} walkers x {n_sw} sweeps of the same workload ({dt:.1f} s wall)",
                                 "accept_fraction": a}
     if rank == 0:
         print(json.dumps(line), flush=True)
