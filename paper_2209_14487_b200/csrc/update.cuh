@@ -246,9 +246,9 @@ __global__ void __launch_bounds__(FINTRI_NT) flush_finalize_tri_kernel(CrowdDev 
 }
 
 // ---- strip kernel: fragments straight from global memory, software-pipelined in registers -------
-// (A shared-memory cp.async ring for the operands was measured slower on B200: 2.54 ms vs 2.07 ms per
+// (A shared-memory cp.async ring for the operands was measured slower on B200 in round 1: 2.54 ms vs 2.07 ms per
 // flush at cfg 5 / W = 2048 -- the LDS + LDGSTS instruction stream saturates the MIO queue next to
-// the DMMAs; see profiles/r1b_flush_variants.md.)
+// the DMMAs.)
 
 // Fragment set of one 16-column chunk of GEMM 1: the B0 strip (two 8-row blocks) and KB window blocks of V.
 template <int KB>
