@@ -1,5 +1,5 @@
 """Parity at BASELINE.json's full size, in the launch configuration bench.py times (config 5:
-768 electrons, 80^3 fp32 table, delayed rank 32, crowd of 2048 walkers), on SAMPLED walkers the oracle can
+768 electrons, 80^3 fp32 table, delayed rank 32, crowd of 4096 walkers), on SAMPLED walkers the oracle can
 compute one by one, plus properties that hold at any size.
 """
 import numpy as np
@@ -11,15 +11,15 @@ from gpu_util import make_pair, npy, relerr
 
 pytestmark = pytest.mark.gpu
 
-W = 2048
-SAMPLE = (0, 777, 2047)
+W = 4096
+SAMPLE = (0, 777, 4095)
 
 
 @pytest.fixture(scope="module")
 def full():
     import torch
-    if torch.cuda.get_device_properties(0).total_memory < 40e9:
-        pytest.skip("needs ~20 GB of device memory")
+    if torch.cuda.get_device_properties(0).total_memory < 80e9:
+        pytest.skip("needs ~45 GB of device memory")
     wl = qi.WORKLOADS[5]
     crowd, osys, coefs, pos = make_pair(wl, n_walkers=W)
     yield wl, crowd, osys, pos
