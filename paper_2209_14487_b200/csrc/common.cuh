@@ -25,7 +25,7 @@ struct CrowdDev {
   unsigned seed_lo, seed_hi;
   int grid[3];
   double tau, sqrt_tau, j2_a, j2_b;
-  double box[3], inv_box[3], inv_h[3];
+  double box[3], inv_box[3], inv_h[3], inv_grid[3];
   unsigned orb_stride_v;  // orbital stride of the table in 16-byte vectors
   unsigned tab_vecs;      // vectors of the table that hold orbitals < orb_stride (per grid point)
   const void* coefs;
@@ -93,6 +93,59 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* sm)
 #pragma unroll
     for (int w = 0; w < NT / 32; ++w) s += sm[w * NV + i];
     v[i] = s;
+  }
+  __syncthreads();
+}
+
+// Sum NV <= 8 values over a block of NT threads; only thread 0 gets the totals (v of the other threads is
+// left undefined).  Within a warp the eight sums are reduced together by a butterfly that halves the number
+// of live values at each of the first three steps (9 double shuffles instead of 40); every partial is the
+// same pairwise tree (xor 16, 8, 4, 2, 1) as warp_sum, so the totals are bit-identical to block_sum's.
+// sm: 8*NT/32 doubles.
+template <int NV, int NT>
+__device__ __forceinline__ void block_sum_t0(double (&v)[NV], double* sm)
+{
+  static_assert(NV <= 8, "block_sum_t0 reduces at most 8 values");
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double a[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) a[i] = i < NV ? v[i] : 0.0;
+  double b[4], c[2], e;
+  {
+    const bool hi = lane & 16;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const double keep = hi ? a[i + 4] : a[i], send = hi ? a[i] : a[i + 4];
+      b[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+  }
+  {
+    const bool hi = lane & 8;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const double keep = hi ? b[i + 2] : b[i], send = hi ? b[i] : b[i + 2];
+      c[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+  }
+  {
+    const bool hi = lane & 4;
+    const double keep = hi ? c[1] : c[0], send = hi ? c[0] : c[1];
+    e = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+  }
+  e += __shfl_xor_sync(0xffffffffu, e, 2);
+  e += __shfl_xor_sync(0xffffffffu, e, 1);
+  // lane now holds quantity q = 4 [bit 4] + 2 [bit 3] + [bit 2]
+  const int q = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+  if ((lane & 3) == 0) sm[warp * 8 + q] = e;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      double s = 0.0;
+#pragma unroll
+      for (int w = 0; w < NT / 32; ++w) s += sm[w * 8 + i];
+      v[i] = s;
+    }
   }
   __syncthreads();
 }

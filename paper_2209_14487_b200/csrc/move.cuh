@@ -180,7 +180,7 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
     j2_partial(d, R, k, rk, v[3], g);
     v[4] = g[0]; v[5] = g[1]; v[6] = g[2];
   }
-  block_sum<7, MOVE_NT>(v, red);
+  block_sum_t0<7, MOVE_NT>(v, red);
   if (!rnew_given && !gauss_pre) {
     if (tid < 5) red[tid] = gauss_piece(d, w, k, tid);
     __syncthreads();
@@ -234,7 +234,7 @@ __device__ __forceinline__ void dev_ratio_grad(const CrowdDev& d, int w, int k, 
     j2_partial(d, R, k, rn, v[4], g);
     v[5] = g[0]; v[6] = g[1]; v[7] = g[2];
   }
-  block_sum<8, MOVE_NT>(v, red);
+  block_sum_t0<8, MOVE_NT>(v, red);
   if (tid == 0) {
     const double rho_d = v[0];
     const double rho_j = exp(v[4] - *ms.usum_old);

@@ -507,6 +507,7 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
     d.box[a] = desc->box[a];
     d.inv_box[a] = 1.0 / desc->box[a];
     d.inv_h[a] = (double)desc->grid[a] / desc->box[a];
+    d.inv_grid[a] = 1.0 / (double)desc->grid[a];
   }
   d.orb_stride_v = (unsigned)(desc->orb_stride / vw);
   d.tab_vecs = d.orb_stride_v;

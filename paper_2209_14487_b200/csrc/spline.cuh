@@ -37,14 +37,17 @@ __device__ __forceinline__ void spline_axis(const CrowdDev& d, int c, double x, 
   const double fl = floor(u);
   const double t = u - fl;
   const double t2 = t * t, t3 = t2 * t, omt = 1.0 - t;
-  s.w[c][0] = (T)(omt * omt * omt / 6.0);
-  s.w[c][1] = (T)((3.0 * t3 - 6.0 * t2 + 4.0) / 6.0);
-  s.w[c][2] = (T)((-3.0 * t3 + 3.0 * t2 + 3.0 * t + 1.0) / 6.0);
-  s.w[c][3] = (T)(t3 / 6.0);
-  s.dw[c][0] = (T)(-omt * omt / 2.0 * ih);
-  s.dw[c][1] = (T)((3.0 * t2 - 4.0 * t) / 2.0 * ih);
-  s.dw[c][2] = (T)((-3.0 * t2 + 2.0 * t + 1.0) / 2.0 * ih);
-  s.dw[c][3] = (T)(t2 / 2.0 * ih);
+  // (multiplications by 1/6 and 1/2: an fp64 division costs ~30 dependent instructions on this serial path)
+  constexpr double sixth = 1.0 / 6.0;
+  const double hih = 0.5 * ih;
+  s.w[c][0] = (T)(omt * omt * omt * sixth);
+  s.w[c][1] = (T)((3.0 * t3 - 6.0 * t2 + 4.0) * sixth);
+  s.w[c][2] = (T)((-3.0 * t3 + 3.0 * t2 + 3.0 * t + 1.0) * sixth);
+  s.w[c][3] = (T)(t3 * sixth);
+  s.dw[c][0] = (T)(-omt * omt * hih);
+  s.dw[c][1] = (T)((3.0 * t2 - 4.0 * t) * hih);
+  s.dw[c][2] = (T)((-3.0 * t2 + 2.0 * t + 1.0) * hih);
+  s.dw[c][3] = (T)(t2 * hih);
   const double ih2 = ih * ih;
   s.d2w[c][0] = (T)(omt * ih2);
   s.d2w[c][1] = (T)((3.0 * t - 2.0) * ih2);
@@ -52,7 +55,7 @@ __device__ __forceinline__ void spline_axis(const CrowdDev& d, int c, double x, 
   s.d2w[c][3] = (T)(t * ih2);
   // (i - 1) mod Ng, floor toward -inf (D:A11); exact in fp64 for |i| < 2^50
   const double a = fl - 1.0;
-  const double q = floor(a / (double)Ng);
+  const double q = floor(a * d.inv_grid[c]);  // may be off by one at exact multiples: fixed up below
   int i0 = (int)(a - q * (double)Ng);
   if (i0 < 0) i0 += Ng;
   if (i0 >= Ng) i0 -= Ng;
@@ -142,22 +145,34 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
 #pragma unroll
         for (int e = 0; e < VW; ++e) out[q][e] = (T)0;
     }
+    // Sum over the four planes (lanes a = 0..3) with the owner of each quantity as the only receiver: lane a ends
+    // up with quantity a, lane 0 also with the laplacian.  Same pairwise tree per value as two full xor-shuffles,
+    // (p_a + p_{a^1}) + (p_{a^2} + p_{a^3}), with 5 instead of 10 shuffles per value.
+    const bool odd = a & 1, up = a & 2;
+    T r0[VW], r1[VW], r2[VW];  // after step 1: even lanes hold q0, q2, q4; odd lanes hold q1, q3 (r2 unused)
 #pragma unroll
-    for (int q = 0; q < 5; ++q)
+    for (int e = 0; e < VW; ++e) {
+      const T s0 = odd ? out[0][e] : out[1][e], s1 = odd ? out[2][e] : out[3][e], s2 = odd ? out[4][e] : (T)0;
+      const T k0 = odd ? out[1][e] : out[0][e], k1 = odd ? out[3][e] : out[2][e], k2 = out[4][e];
+      r0[e] = k0 + shfl_xor_t(s0, 1);
+      r1[e] = k1 + shfl_xor_t(s1, 1);
+      r2[e] = k2 + shfl_xor_t(s2, 1);
+    }
+    T f0[VW], f1[VW];  // after step 2: lane 0: q0, q4; lane 1: q1; lane 2: q2; lane 3: q3
 #pragma unroll
-      for (int e = 0; e < VW; ++e) {
-        T v = out[q][e];
-        v += shfl_xor_t(v, 1);
-        v += shfl_xor_t(v, 2);
-        out[q][e] = ((int)(chunk * VW) + e < d.M) ? v : (T)0;
-      }
+    for (int e = 0; e < VW; ++e) {
+      const T s0 = up ? r0[e] : r1[e], s1 = up ? r2[e] : (T)0;
+      const T k0 = up ? r1[e] : r0[e], k1 = r2[e];
+      f0[e] = k0 + shfl_xor_t(s0, 2);
+      f1[e] = k1 + shfl_xor_t(s1, 2);
+    }
+#pragma unroll
+    for (int e = 0; e < VW; ++e)
+      if ((int)(chunk * VW) + e >= d.M) f0[e] = f1[e] = (T)0;
     if (chunk < chunks) {
       T* o = vgl + (size_t)chunk * VW;
-      // lane a stores quantity a; lane 0 also stores the laplacian
-      if (a == 0) { st16(o, out[0]); st16(o + (size_t)4 * d.ns, out[4]); }
-      else if (a == 1) st16(o + (size_t)d.ns, out[1]);
-      else if (a == 2) st16(o + (size_t)2 * d.ns, out[2]);
-      else st16(o + (size_t)3 * d.ns, out[3]);
+      st16(o + (size_t)a * d.ns, f0);
+      if (a == 0) st16(o + (size_t)4 * d.ns, f1);
     }
   }
 }
