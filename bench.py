@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--crowd-sweep", action="store_true", help="also print moves/s vs crowd size and delay rank")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sub-crowds", type=int, default=None, help="sub-crowds qmc_sweep runs on separate streams (1..4)")
     ap.add_argument("--no-probes", action="store_true", help="skip the step-call / rank-1 kernel probes")
     ap.add_argument("--ref-walkers", type=int, default=None, help="walkers of the oracle sample (default = cores)")
     return ap.parse_args()
@@ -283,6 +284,8 @@ def run_cuda(args):
     crowd, pos = make_crowd(wl, W, kd, id0, coefs_dev, dev)
     torch.cuda.synchronize()
     create_s = time.perf_counter() - t0
+    if args.sub_crowds:
+        crowd.set_option(q.QMC_OPT_SUBCROWDS, args.sub_crowds)
 
     with ClockSampler(local_rank) as clk:
         ms, proposed, accepted, launches = time_sweeps(crowd, args.steps, max(args.warmup, 0), sync_all)

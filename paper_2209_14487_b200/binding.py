@@ -16,6 +16,7 @@ _lib = None
 QMC_OK, QMC_ERR_INVALID_ARG, QMC_ERR_CUDA, QMC_ERR_WORKSPACE, QMC_ERR_SINGULAR, QMC_ERR_STATE = range(6)
 QMC_OPT_GRAPH = 0
 QMC_OPT_PROFILE = 1
+QMC_OPT_SUBCROWDS = 2
 KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush", "ratio_accept",
                   "fused_move", "window")
 

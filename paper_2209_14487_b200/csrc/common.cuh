@@ -22,6 +22,7 @@ struct CrowdDev {
   int W, N, n, M, ns;
   int kd, kdp;
   int walker_id0;
+  int w0;  // first walker of this launch (sub-crowds of qmc_sweep run on two streams; 0 otherwise)
   unsigned seed_lo, seed_hi;
   int grid[3];
   double tau, sqrt_tau, j2_a, j2_b;

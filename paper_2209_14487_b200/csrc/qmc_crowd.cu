@@ -66,6 +66,9 @@ struct qmc_crowd {
   uint64_t proposed, flushes, launches;
   uint32_t sweep_host;
   int use_graph;
+  int n_sub;                        // sub-crowds of qmc_sweep (delay_rank > 1), each on its own stream
+  cudaStream_t sub_stream[4];
+  cudaEvent_t ev_fork, ev_join[4];
   uint64_t graph_launches, graph_flushes;  // per replay of the captured sweep
   cudaGraphExec_t graph_exec;
   // QMC_OPT_PROFILE: CUDA-event pairs around every kernel of the plain-launch sweep
@@ -302,44 +305,40 @@ int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
   return QMC_OK;
 }
 
-int launch_flush(qmc_crowd* c, int spin, bool from_window = false)
+template <int KDP>
+void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cudaStream_t st)
 {
-  const CrowdDev& d = c->dev;
   const int rows_per_cta = (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP;
-  dim3 grid((d.ns + rows_per_cta - 1) / rows_per_cta, d.W);
+  dim3 grid((d.ns + rows_per_cta - 1) / rows_per_cta, wn);
+  if (from_window) {
+    flush_finalize_tri_kernel<KDP><<<wn, FINTRI_NT, (size_t)KDP * (KDP + 1) * 8, st>>>(d);
+  } else {
+    const int fcols = FINALIZE_NT / (KDP > 32 ? KDP / 32 : 1);
+    dim3 fgrid((d.ns + fcols - 1) / fcols, wn);
+    flush_finalize_kernel<KDP><<<fgrid, FINALIZE_NT, (size_t)KDP * KDP * 8, st>>>(d, spin);
+  }
+  flush_kernel<KDP / 8><<<grid, FLUSH_NT, 0, st>>>(d, spin);
+}
+
+// Flush of walkers [w0, w0 + wn) on stream st (the whole crowd on the crowd's stream by default).
+int launch_flush(qmc_crowd* c, int spin, bool from_window = false, int w0 = 0, int wn = -1, cudaStream_t st = nullptr)
+{
+  CrowdDev d = c->dev;
+  if (wn < 0) { wn = d.W; st = c->stream; }
+  d.w0 = w0;
   ProfScope ps(c, QMC_K_FLUSH);
-  const int fcols = FINALIZE_NT / (d.kdp > 32 ? d.kdp / 32 : 1);
-  dim3 fgrid((d.ns + fcols - 1) / fcols, d.W);
-  const size_t fsm = (size_t)d.kdp * d.kdp * 8, tsm = (size_t)d.kdp * (d.kdp + 1) * 8;
-  const size_t flush_smem = 0;
   switch (d.kdp) {
-    case 8:
-      if (from_window) flush_finalize_tri_kernel<8><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
-      else flush_finalize_kernel<8><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
-      flush_kernel<1><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
-      break;
-    case 16:
-      if (from_window) flush_finalize_tri_kernel<16><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
-      else flush_finalize_kernel<16><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
-      flush_kernel<2><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
-      break;
-    case 32:
-      if (from_window) flush_finalize_tri_kernel<32><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
-      else flush_finalize_kernel<32><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
-      flush_kernel<4><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
-      break;
-    case 64:
-      if (from_window) flush_finalize_tri_kernel<64><<<d.W, FINTRI_NT, tsm, c->stream>>>(d);
-      else flush_finalize_kernel<64><<<fgrid, FINALIZE_NT, fsm, c->stream>>>(d, spin);
-      flush_kernel<8><<<grid, FLUSH_NT, flush_smem, c->stream>>>(d, spin);
-      break;
+    case 8: launch_flush_kdp<8>(d, spin, from_window, wn, st); break;
+    case 16: launch_flush_kdp<16>(d, spin, from_window, wn, st); break;
+    case 32: launch_flush_kdp<32>(d, spin, from_window, wn, st); break;
+    case 64: launch_flush_kdp<64>(d, spin, from_window, wn, st); break;
     default: return fail(QMC_ERR_INVALID_ARG, "unsupported padded delay rank %d", d.kdp);
   }
   ++c->launches;
   LAUNCH_CHECK(c);
-  CUDA_TRY(cudaMemsetAsync(d.mwin, 0, (size_t)d.W * 4, c->stream));
+  CUDA_TRY(cudaMemsetAsync(d.mwin + w0, 0, (size_t)wn * 4, st));
   ++c->launches;
-  ++c->flushes;
+  if (w0 == 0) ++c->flushes;
   return QMC_OK;
 }
 
@@ -377,10 +376,12 @@ int launch_ratio_accept_t(qmc_crowd* c, int k)
 size_t window_smem(const CrowdDev& d, size_t elem) { return (size_t)win_layout(d.N, d.ns, d.kdp, (int)elem).total * 8; }
 
 template <typename T>
-int launch_window_t(qmc_crowd* c, int k0, int cnt)
+int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t st)
 {
   ProfScope ps(c, QMC_K_WINDOW);
-  window_kernel<T><<<c->dev.W, MOVE_NT, window_smem(c->dev, sizeof(T)), c->stream>>>(c->dev, k0, cnt);
+  CrowdDev d = c->dev;
+  d.w0 = w0;
+  window_kernel<T><<<wn, MOVE_NT, window_smem(d, sizeof(T)), st>>>(d, k0, cnt);
   LAUNCH_CHECK(c);
   return QMC_OK;
 }
@@ -394,14 +395,32 @@ int sweep_once(qmc_crowd* c)
   const CrowdDev& d = c->dev;
   int st = QMC_OK;
   if (d.kd > 1) {
-    for (int spin = 0; spin < 2; ++spin)
-      for (int kk0 = 0; kk0 < d.n; kk0 += d.kd) {
-        const int cnt = d.n - kk0 < d.kd ? d.n - kk0 : d.kd;
-        st = c->is_f64 ? launch_window_t<double>(c, spin * d.n + kk0, cnt) : launch_window_t<float>(c, spin * d.n + kk0, cnt);
-        if (st) return st;
-        st = launch_flush(c, spin, true);
-        if (st) return st;
+    // Walkers never interact, so the crowd may advance as independent sub-crowds (the paper's crowds on separate
+    // streams, Alg. 4 / P:135): with two of them the DMMA-bound flush of one overlaps the window kernel of the other.
+    // Each sub-crowd is in lock-step with itself; results do not depend on the split (same walkers, same counters).
+    const int nsub = (c->n_sub > 1 && !c->profile && d.W >= 2 * c->n_sub) ? c->n_sub : 1;
+    cudaStream_t s0 = c->stream;
+    if (nsub > 1) {
+      CUDA_TRY(cudaEventRecord(c->ev_fork, s0));
+      for (int i = 1; i < nsub; ++i) CUDA_TRY(cudaStreamWaitEvent(c->sub_stream[i], c->ev_fork, 0));
+    }
+    for (int i = 0; i < nsub; ++i) {
+      const int w0 = (int)((long long)d.W * i / nsub), w1 = (int)((long long)d.W * (i + 1) / nsub);
+      cudaStream_t ss = i == 0 ? s0 : c->sub_stream[i];
+      for (int spin = 0; spin < 2; ++spin)
+        for (int kk0 = 0; kk0 < d.n; kk0 += d.kd) {
+          const int cnt = d.n - kk0 < d.kd ? d.n - kk0 : d.kd;
+          st = c->is_f64 ? launch_window_t<double>(c, spin * d.n + kk0, cnt, w0, w1 - w0, ss)
+                         : launch_window_t<float>(c, spin * d.n + kk0, cnt, w0, w1 - w0, ss);
+          if (st) return st;
+          st = launch_flush(c, spin, true, w0, w1 - w0, ss);
+          if (st) return st;
+        }
+      if (i > 0) {
+        CUDA_TRY(cudaEventRecord(c->ev_join[i], ss));
+        CUDA_TRY(cudaStreamWaitEvent(s0, c->ev_join[i], 0));
       }
+    }
     bump_sweep_kernel<<<1, 1, 0, c->stream>>>(d.sweep);
     LAUNCH_CHECK(c);
     return QMC_OK;
@@ -488,6 +507,9 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   c->proposed = c->flushes = c->launches = 0;
   c->sweep_host = 0;
   c->use_graph = 1;
+  c->n_sub = 1;
+  for (int i = 0; i < 4; ++i) { c->sub_stream[i] = nullptr; c->ev_join[i] = nullptr; }
+  c->ev_fork = nullptr;
   c->graph_launches = c->graph_flushes = 0;
   c->graph_exec = nullptr;
   c->profile = 0;
@@ -514,12 +536,19 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   d.coefs = desc->coefs;
   carve(desc, &d, (char*)desc->workspace);
 
-  auto bail = [&](int code) { delete c; return code; };
+  auto bail = [&](int code) { qmc_crowd_destroy(c); return code; };
   cudaError_t e = cudaMemsetAsync(desc->workspace, 0, need, c->stream);
   if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "workspace memset: %s", cudaGetErrorString(e)));
   e = cudaMemcpyAsync(d.R, pos_dev, (size_t)d.W * d.N * 3 * 8, cudaMemcpyDeviceToDevice, c->stream);
   if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "position copy: %s", cudaGetErrorString(e)));
   c->launches += 2;
+  for (int i = 1; i < 4; ++i) {
+    if (cudaStreamCreateWithFlags(&c->sub_stream[i], cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming) != cudaSuccess)
+      return bail(fail(QMC_ERR_CUDA, "sub-crowd stream: %s", cudaGetErrorString(cudaGetLastError())));
+  }
+  if (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess)
+    return bail(fail(QMC_ERR_CUDA, "sub-crowd event: %s", cudaGetErrorString(cudaGetLastError())));
   {
     const int sm = (int)move_smem(d), wsm = (int)window_smem(d, c->elem);
     if (wsm > 227 * 1024 || sm > 227 * 1024)
@@ -550,6 +579,11 @@ int qmc_crowd_destroy(qmc_crowd_t* c)
   if (!c) return QMC_OK;
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  for (int i = 1; i < 4; ++i) {
+    if (c->sub_stream[i]) cudaStreamDestroy(c->sub_stream[i]);
+    if (c->ev_join[i]) cudaEventDestroy(c->ev_join[i]);
+  }
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   delete c;
   return QMC_OK;
 }
@@ -841,6 +875,12 @@ int qmc_crowd_set_option(qmc_crowd_t* c, int option, int value)
   if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
   if (option == QMC_OPT_GRAPH) { c->use_graph = value ? 1 : 0; return QMC_OK; }
   if (option == QMC_OPT_PROFILE) { c->profile = value ? 1 : 0; return QMC_OK; }
+  if (option == QMC_OPT_SUBCROWDS) {
+    if (value < 1 || value > 4) return fail(QMC_ERR_INVALID_ARG, "sub-crowds must be in [1,4]");
+    c->n_sub = value;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    return QMC_OK;
+  }
   return fail(QMC_ERR_INVALID_ARG, "unknown option %d", option);
 }
 

@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d,
   constexpr int LH = KDP / ZL;
   constexpr int COLS = FINALIZE_NT / LH;
   extern __shared__ double s_sinv[];
-  const int w = blockIdx.y;
+  const int w = blockIdx.y + d.w0;
   const int m = d.mwin[w];
   if (m == 0) return;
   const int ns = d.ns;
@@ -217,7 +217,7 @@ __global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize
 {
   constexpr int KB = KDP / 8, SS = KDP + 1;
   extern __shared__ double s_n[];
-  const int w = blockIdx.x;
+  const int w = blockIdx.x + d.w0;
   const int m = d.mwin[w];
   if (m == 0) return;
   const int ns = d.ns, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
@@ -373,7 +373,7 @@ __device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double
 template <int KB>
 __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(CrowdDev d, int spin)
 {
-  const int w = blockIdx.y;
+  const int w = blockIdx.y + d.w0;
   const int m = d.mwin[w];
   if (m == 0) return;
   const int ns = d.ns, kdp = d.kdp;

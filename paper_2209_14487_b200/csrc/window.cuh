@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(Crowd
 {
   extern __shared__ double sm[];
   __shared__ SplineW<T> sw;
-  const int w = blockIdx.x, ns = d.ns, kdp = d.kdp, tid = threadIdx.x;
+  const int w = blockIdx.x + d.w0, ns = d.ns, kdp = d.kdp, tid = threadIdx.x;
   const WinLayout L = win_layout(d.N, ns, kdp, (int)sizeof(T));
   double* R_s = sm + L.R;
   double* b_s = sm + L.b;    // row of the current move

@@ -172,3 +172,23 @@ def test_sweep_host_equals_set_positions_plus_sweep():
     assert np.array_equal(host.numpy(), npy(b.positions()))
     assert np.array_equal(npy(a.positions()), host.numpy())
     assert stats == b.stats()
+
+
+def test_sub_crowds_on_separate_streams_do_not_change_results():
+    """QMC_OPT_SUBCROWDS: qmc_sweep advances the crowd as independent sub-crowds on separate streams (PAPER.md:135);
+    walkers are independent and counters are global, so every split gives bit-identical state."""
+    import paper_2209_14487_b200 as q
+    wl = qi.small_workload(n_elec=48, grid=10, box=6.0, coef_dtype="f32", coef_dist="normal", n_walkers=11, tau=0.02,
+                           delay_rank=8, cfg=15)
+    ref, _, _, _ = make_pair(wl)
+    ref.qmc_sweep(2)
+    for nsub, graph in ((2, 1), (3, 0), (4, 1)):
+        c, _, _, _ = make_pair(wl)
+        c.set_option(q.QMC_OPT_GRAPH, graph)
+        c.set_option(q.QMC_OPT_SUBCROWDS, nsub)
+        c.qmc_sweep(1)
+        c.qmc_sweep(1)
+        assert np.array_equal(npy(c.positions()), npy(ref.positions()))
+        for spin in (0, 1):
+            assert np.array_equal(npy(c.inverse(spin)), npy(ref.inverse(spin)))
+        assert c.stats() == ref.stats()
