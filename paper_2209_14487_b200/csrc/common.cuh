@@ -98,8 +98,8 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* sm)
   __syncthreads();
 }
 
-// Sum NV <= 8 values over a block of NT threads; only thread 0 gets the totals (v of the other threads is
-// left undefined).  Within a warp the eight sums are reduced together by a butterfly that halves the number
+// Sum NV <= 8 values over a block of NT threads; only threads 0, 1, 2 get the totals (v of the other threads
+// is left undefined).  Within a warp the eight sums are reduced together by a butterfly that halves the number
 // of live values at each of the first three steps (9 double shuffles instead of 40); every partial is the
 // same pairwise tree (xor 16, 8, 4, 2, 1) as warp_sum, so the totals are bit-identical to block_sum's.
 // sm: 8*NT/32 doubles.
@@ -139,7 +139,7 @@ __device__ __forceinline__ void block_sum_t0(double (&v)[NV], double* sm)
   const int q = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
   if ((lane & 3) == 0) sm[warp * 8 + q] = e;
   __syncthreads();
-  if (threadIdx.x == 0) {
+  if (threadIdx.x < 3) {
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
       double s = 0.0;

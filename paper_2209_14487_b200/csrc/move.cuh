@@ -159,11 +159,12 @@ __device__ __forceinline__ double gauss_piece(const CrowdDev& d, int w, int k, i
 // Delta = fl32(tau G + sqrt(tau) chi), r' = r_k + Delta, chi by Box-Muller      (D:C4, C7)
 // b_s: the inverse row of electron k with the window applied (shared memory); cache: [4][ns] of
 // electron k; R: positions [N][3] of the walker.  The five transcendental pieces of the Gaussians
-// run on five threads (or arrive precomputed in gauss_pre[5]).  Results go to ms (thread 0); callers synchronise before reading them.
+// run on five threads (or arrive precomputed in gauss_pre[5]).  Threads 0..2 take one component each, write the
+// results to ms and, if sw_out is given, the spline weights of their axis at r'; callers synchronise before reading.
 template <typename T>
 __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k, const double* b_s, const T* cache,
                                                  const double* R, const double* rnew_given, MoveScal ms, double* red,
-                                                 const double* gauss_pre = nullptr)
+                                                 const double* gauss_pre = nullptr, SplineW<T>* sw_out = nullptr)
 {
   const int ns = d.ns, tid = threadIdx.x;
   // v[0..2] = b . grad phi(r_k), v[3] = usum_old, v[4..6] = grad_k ln Psi_J(R)
@@ -186,28 +187,25 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
     __syncthreads();
   }
   const double* gp = gauss_pre ? gauss_pre : red;
-  if (tid == 0) {
-    const double g_old[3] = {v[0] + v[4], v[1] + v[5], v[2] + v[6]};
-    double delta[3], rn[3];
+  if (tid < 3) {  // one thread per component: G, chi, Delta, r', and (window kernel) the spline weights of that axis
+    const int c = tid;
+    const double g_old = c == 0 ? v[0] + v[4] : (c == 1 ? v[1] + v[5] : v[2] + v[6]);
+    const double rkc = R[3 * k + c];
+    double delta, rn;
     if (rnew_given) {
-#pragma unroll
-      for (int c = 0; c < 3; ++c) { rn[c] = rnew_given[3 * (size_t)w + c]; delta[c] = rn[c] - rk[c]; }
+      rn = rnew_given[3 * (size_t)w + c];
+      delta = rn - rkc;
     } else {
-      const double chi[3] = {gp[0] * gp[1], gp[0] * gp[2], gp[3] * gp[4]};
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        const double xx = __dadd_rn(__dmul_rn(d.tau, g_old[c]), __dmul_rn(d.sqrt_tau, chi[c]));
-        delta[c] = (double)__double2float_rn(xx);
-        rn[c] = rk[c] + delta[c];
-      }
+      const double chi = c == 0 ? gp[0] * gp[1] : (c == 1 ? gp[0] * gp[2] : gp[3] * gp[4]);
+      const double xx = __dadd_rn(__dmul_rn(d.tau, g_old), __dmul_rn(d.sqrt_tau, chi));
+      delta = (double)__double2float_rn(xx);
+      rn = rkc + delta;
     }
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      ms.g_old[c] = g_old[c];
-      ms.delta[c] = delta[c];
-      ms.rn[c] = rn[c];
-    }
-    *ms.usum_old = v[3];
+    ms.g_old[c] = g_old;
+    ms.delta[c] = delta;
+    ms.rn[c] = rn;
+    if (c == 0) *ms.usum_old = v[3];
+    if (sw_out) spline_axis<T>(d, c, rn, *sw_out);
   }
 }
 

@@ -68,19 +68,26 @@ __device__ __forceinline__ void spline_axis(const CrowdDev& d, int c, double x, 
   }
 }
 
-// Contribution of x-plane a to the five quantities of one 16-byte orbital slice `chunk`.
-// out[0] = phi, out[1..3] = d/dx, d/dy, d/dz, out[4] = laplacian.
+// The 16 stencil rows (4 y x 4 z) of x-plane a for one 16-byte orbital slice `chunk`: 16 independent loads.
 template <typename T>
-__device__ __forceinline__ void spline_plane(const T* __restrict__ tab, const SplineW<T>& s, int a, unsigned chunk,
-                                             T (&out)[5][Vec16<T>::W])
+__device__ __forceinline__ void spline_plane_load(const T* __restrict__ tab, const SplineW<T>& s, int a, unsigned chunk,
+                                                  T (&p)[4][4][Vec16<T>::W])
 {
   constexpr int VW = Vec16<T>::W;
   const unsigned base = s.off[0][a] + chunk;
-  T p[4][4][VW];
 #pragma unroll
   for (int b = 0; b < 4; ++b)
 #pragma unroll
     for (int c = 0; c < 4; ++c) ld16(tab + (size_t)(base + s.off[1][b] + s.off[2][c]) * VW, p[b][c]);
+}
+
+// Contribution of x-plane a to the five quantities of the slice, from its 16 loaded rows.
+// out[0] = phi, out[1..3] = d/dx, d/dy, d/dz, out[4] = laplacian.
+template <typename T>
+__device__ __forceinline__ void spline_plane_sum(const SplineW<T>& s, int a, const T (&p)[4][4][Vec16<T>::W],
+                                                 T (&out)[5][Vec16<T>::W])
+{
+  constexpr int VW = Vec16<T>::W;
   T u00[VW], u10[VW], u20[VW], u01[VW], u02[VW];
 #pragma unroll
   for (int e = 0; e < VW; ++e) u00[e] = u10[e] = u20[e] = u01[e] = u02[e] = (T)0;
@@ -119,18 +126,20 @@ __device__ __forceinline__ double shfl_xor_t(double v, int m) { return __shfl_xo
 // All orbitals at position r by the whole CTA (NT threads, NT % 32 == 0).  `s` is shared memory;
 // `vgl` (global or shared) receives [5][ns]: phi, d/dx, d/dy, d/dz, laplacian, zero beyond M.
 // Contains two __syncthreads(); must be called by all threads of the CTA.
-// `side(tid)` runs on the threads of warps >= 1 while three threads of warp 0 build the weights
-// (a slot for work that is off the caller's critical path).
+// `side(tid)` runs on the threads of warps >= 1 right after the first round of loads has been issued, i.e. under
+// their DRAM latency (a slot for work that is off the caller's critical path).
 struct NoSideWork { __device__ __forceinline__ void operator()(int) const {} };
+// r == nullptr: the caller has already filled `s` for this position (spline_axis per axis).
 template <typename T, int NT, typename Side = NoSideWork>
 __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, SplineW<T>& s, T* vgl, Side side = Side())
 {
   constexpr int VW = Vec16<T>::W;
   const int tid = threadIdx.x, a = tid & 3, g = tid >> 2;
-  __syncthreads();  // previous users of `s` are done
-  if (tid < 3) spline_axis<T>(d, tid, r[tid], s);
-  else if (tid >= 32) side(tid);
-  __syncthreads();
+  __syncthreads();  // previous users of `s` are done / the caller's weights are visible
+  if (r) {
+    if (tid < 3) spline_axis<T>(d, tid, r[tid], s);
+    __syncthreads();
+  }
   const T* tab = static_cast<const T*>(d.coefs);
   const unsigned chunks = (unsigned)d.ns / VW;
 #pragma unroll 1
@@ -138,8 +147,12 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
     const unsigned chunk = c0 + g;
     T out[5][VW];
     if (chunk < d.tab_vecs && chunk < chunks) {
-      spline_plane<T>(tab, s, a, chunk, out);
+      T p[4][4][VW];
+      spline_plane_load<T>(tab, s, a, chunk, p);
+      if (c0 == 0 && tid >= 32) side(tid);
+      spline_plane_sum<T>(s, a, p, out);
     } else {
+      if (c0 == 0 && tid >= 32) side(tid);
 #pragma unroll
       for (int q = 0; q < 5; ++q)
 #pragma unroll

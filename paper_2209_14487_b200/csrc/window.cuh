@@ -201,8 +201,8 @@ __global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(Crowd
       cp_async_cta(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
     }
     // ---- G_k(R), proposal, orbitals at r' (the next move's Gaussians ride along), ratio, decision ----
-    dev_gold_propose<T>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss);
-    spline_cta<T, MOVE_NT>(d, ms.rn, sw, vgl_s, [&](int t) {
+    dev_gold_propose<T>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss, &sw);
+    spline_cta<T, MOVE_NT>(d, nullptr, sw, vgl_s, [&](int t) {
       if (more && t < 37) gauss[t - 32] = gauss_piece(d, w, k + 1, t - 32);
     });
     __syncthreads();
