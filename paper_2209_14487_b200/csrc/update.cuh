@@ -102,6 +102,9 @@ __global__ void __launch_bounds__(RANK1_NT) rank1_generic_kernel(CrowdDev d, int
   }
 }
 
+#ifndef QMC_FLUSH_PFD1
+#define QMC_FLUSH_PFD1 0
+#endif
 #ifndef QMC_FLUSH_PFD
 #define QMC_FLUSH_PFD 8
 #endif
@@ -276,6 +279,16 @@ __global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize
   }
 }
 
+// Measured alternatives on B200 (cfg 5, W = 4096, round 1):
+//  - the DMMA.8x8x4 issue ceiling with this chain structure is 37.2 TFLOP/s, and 34.4 TFLOP/s with the V and strip
+//    fragments loaded straight from L1/L2 as here -- the operand path is not the limit, DRAM streaming is: the strip is
+//    read twice and the second read misses L2 half the time (13.8 GB of traffic for 9.7 GB algorithmic; skipping the
+//    second read shortens the flush by 0.85 ms);
+//  - L2 eviction hints (QMC_FLUSH_L2HINT) with or without a persisting-L2 set-aside: no gain (the set-aside slows the
+//    window kernel);
+//  - a K-split form (eight warps share a strip, each keeps its columns in registers, partial products summed through
+//    shared memory, strip read once: 10.3 GB of traffic) ran at 5.0 ms instead of 3.3 ms: two block barriers per strip
+//    and eight warps per SM leave the DMMA pipe 42 % busy.
 // ---- strip kernel: fragments straight from global memory, software-pipelined in registers -------
 // (A shared-memory cp.async ring for the operands was measured slower on B200 in round 1: 2.54 ms vs 2.07 ms per
 // flush at cfg 5 / W = 2048 -- the LDS + LDGSTS instruction stream saturates the MIO queue next to
@@ -297,6 +310,12 @@ __device__ __forceinline__ void load_frag1(Frag1<KB>& f, const double* a0p, cons
   if ((threadIdx.x & 3) == 0 && s + 16 * QMC_FLUSH_PFD < ns) {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(a0p + s + 16 * QMC_FLUSH_PFD));
     asm volatile("prefetch.global.L2 [%0];" ::"l"(a1p + s + 16 * QMC_FLUSH_PFD));
+  }
+#endif
+#if QMC_FLUSH_PFD1 > 0
+  if ((threadIdx.x & 3) == 0 && s + 16 * QMC_FLUSH_PFD1 < ns) {
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(a0p + s + 16 * QMC_FLUSH_PFD1));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(a1p + s + 16 * QMC_FLUSH_PFD1));
   }
 #endif
 #pragma unroll
