@@ -288,7 +288,8 @@ __global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize
 //    window kernel);
 //  - a K-split form (eight warps share a strip, each keeps its columns in registers, partial products summed through
 //    shared memory, strip read once: 10.3 GB of traffic) ran at 5.0 ms instead of 3.3 ms: two block barriers per strip
-//    and eight warps per SM leave the DMMA pipe 42 % busy.
+//    and eight warps per SM leave the DMMA pipe 42 % busy;
+//  - 8-row strips (half the L2 reuse distance, twice the V fragment traffic per DMMA): 4.1 ms instead of 3.7 ms.
 // ---- strip kernel: fragments straight from global memory, software-pipelined in registers -------
 // (A shared-memory cp.async ring for the operands was measured slower on B200 in round 1: 2.54 ms vs 2.07 ms per
 // flush at cfg 5 / W = 2048 -- the LDS + LDGSTS instruction stream saturates the MIO queue next to
