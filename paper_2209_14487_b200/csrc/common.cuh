@@ -60,6 +60,25 @@ __device__ __forceinline__ void ld16(const double* p, double (&v)[2])
   const double2 q = __ldg(reinterpret_cast<const double2*>(p));
   v[0] = q.x; v[1] = q.y;
 }
+// Streaming 16-byte loads of read-only data with an L2 evict-first policy (the spline table is gathered once per
+// move and must not push the per-walker state out of L2: window kernel 4.94 -> 4.63 ms at cfg 5, W = 4096; an
+// evict_last policy on the walker's own block rows, tried on top, was slightly slower and is not used).
+// pol: createpolicy.fractional.L2::evict_first.
+__device__ __forceinline__ unsigned long long l2_evict_first_policy()
+{
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void ld16_stream(const float* p, float (&v)[4], unsigned long long pol)
+{
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "l"(p), "l"(pol));
+}
+__device__ __forceinline__ void ld16_stream(const double* p, double (&v)[2], unsigned long long pol)
+{
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v[0]), "=d"(v[1]) : "l"(p), "l"(pol));
+}
 __device__ __forceinline__ void st16(float* p, const float (&v)[4])
 {
   *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
