@@ -65,6 +65,8 @@ def lib():
     L.oracle_j2_logpsi.argtypes = [C.POINTER(System), dp]
     L.oracle_j2_logpsi.restype = C.c_double
     L.oracle_j2_usum_grad.argtypes = [C.POINTER(System), dp, C.c_int, dp, dp, dp]
+    L.oracle_kinetic_energy.argtypes = [C.POINTER(System), dp, dp, dp, dp]
+    L.oracle_kinetic_energy.restype = C.c_double
     L.oracle_lu_inverse_transpose.argtypes = [C.c_int, dp, dp, dp, C.POINTER(C.c_int)]
     L.oracle_sm_update.argtypes = [C.c_int, dp, C.c_int, dp, C.c_double]
     ip = C.POINTER(C.c_int32)
@@ -161,6 +163,16 @@ class OracleSystem:
         us, g = C.c_double(), np.zeros(3)
         lib().oracle_j2_usum_grad(self.ref, _dp(R), k, _dp(rk), C.byref(us), _dp(g))
         return us.value, g
+
+
+    def kinetic_energy(self, R, B_up, B_dn):
+        """(T, per-electron terms): -1/2 sum_k lap_k Psi / Psi at R with the transposed inverses B_up, B_dn."""
+        R, B_up, B_dn = _f64(R), _f64(B_up), _f64(B_dn)
+        n = self.n_elec // 2
+        assert R.shape == (self.n_elec, 3) and B_up.shape == (n, n) and B_dn.shape == (n, n)
+        e = np.zeros(self.n_elec)
+        t = lib().oracle_kinetic_energy(self.ref, _dp(R), _dp(B_up), _dp(B_dn), _dp(e))
+        return float(t), e
 
 
 def bspline_weights(t: float):

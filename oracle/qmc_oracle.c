@@ -199,6 +199,53 @@ void oracle_j2_usum_grad(const oracle_system* s, const double* R, int k, const d
   grad[0] = g[0]; grad[1] = g[1]; grad[2] = g[2];
 }
 
+/* Kinetic part of the local energy (Alg. 1 line 11), atomic units:
+ *   T(R) = -1/2 sum_k lap_k Psi / Psi,      lap_k Psi / Psi = lap_k ln Psi + |grad_k ln Psi|^2,
+ * with ln Psi = ln D_up + ln D_dn + ln Psi_J (C4).  For electron k of spin block sigma, row b = B^sigma[k,:] of
+ * the transposed inverse (C2) and the orbitals at r_k:
+ *   grad_k ln D = sum_j b_j grad phi_j,     lap_k ln D = sum_j b_j lap phi_j - |grad_k ln D|^2,
+ *   grad_k ln Psi_J = sum_{i!=k} u'(r) d/r,  lap_k ln Psi_J = sum_{i!=k} [u''(r) + 2 u'(r)/r],
+ *   u = a r/(1 + b r), u' = a/(1 + b r)^2, u'' = -2 a b/(1 + b r)^3 (C3).
+ * B_up, B_dn: [n][n] transposed inverses at R; e_elec: [N] per-electron terms or NULL.  Returns T. */
+double oracle_kinetic_energy(const oracle_system* s, const double* R, const double* B_up, const double* B_dn,
+                             double* e_elec)
+{
+  const int N = s->n_elec, n = N / 2, M = s->n_orb;
+  double* phi = (double*)malloc(sizeof(double) * 5 * (size_t)M);
+  double* dph = phi + M;
+  double* d2ph = phi + 4 * (size_t)M;
+  double total = 0.0;
+  for (int k = 0; k < N; ++k) {
+    const double* b = (k < n ? B_up : B_dn) + (size_t)(k % n) * n;
+    oracle_spo_vgl(s, R + 3 * k, phi, dph, d2ph);
+    double gd[3] = { 0.0, 0.0, 0.0 }, ld = 0.0;
+    for (int j = 0; j < M; ++j) {
+      for (int c = 0; c < 3; ++c) gd[c] += b[j] * dph[(size_t)c * M + j];
+      ld += b[j] * d2ph[j];
+    }
+    double lap_ln_d = ld - (gd[0] * gd[0] + gd[1] * gd[1] + gd[2] * gd[2]);
+    double gj[3] = { 0.0, 0.0, 0.0 }, lap_ln_j = 0.0, d[3];
+    for (int i = 0; i < N; ++i) {
+      if (i == k) continue;
+      double r = min_image_dist(s, R + 3 * k, R + 3 * i, d);
+      if (r > 0.0) {
+        double den = 1.0 + s->j2_b * r;
+        double du = s->j2_a / (den * den);
+        double d2u = -2.0 * s->j2_a * s->j2_b / (den * den * den);
+        for (int c = 0; c < 3; ++c) gj[c] += du * d[c] / r;
+        lap_ln_j += d2u + 2.0 * du / r;
+      }
+    }
+    double g2 = 0.0;
+    for (int c = 0; c < 3; ++c) g2 += (gd[c] + gj[c]) * (gd[c] + gj[c]);
+    double ek = -0.5 * (lap_ln_d + lap_ln_j + g2);
+    if (e_elec) e_elec[k] = ek;
+    total += ek;
+  }
+  free(phi);
+  return total;
+}
+
 /* ------------------------------------------------------------------------------------
  * LU with partial pivoting (Doolittle, row swaps), in place on a copy. Returns 0, or 4
  * (= "singular") when a pivot is zero or non-finite (A16).

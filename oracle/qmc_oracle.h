@@ -29,6 +29,8 @@
  *   SM / delayed .. full re-inversion (numpy) after every accepted move / flush
  *   Jastrow ....... two-electron closed form, full pair-sum difference, finite differences
  *   accept rule ... tau->0 limit, constant-orbital case, sampling of |phi|^2 (histogram)
+ *   kinetic ....... central second differences of the brute-force Psi = det det exp(J) (numpy) on tiny systems;
+ *                   free-particle and two-electron Jastrow closed forms
  *   whole sweep ... every logged move re-derived from brute-force determinants; the
  *                   paper prints no worked trajectory, so the *trajectory itself* is
  *                   "parity unpinned" by the paper (S8c T9) and pinned only through
@@ -86,6 +88,10 @@ void oracle_spo_vgl(const oracle_system* sys, const double r[3],
 double oracle_j2_logpsi(const oracle_system* sys, const double* R /*[N][3]*/);
 void   oracle_j2_usum_grad(const oracle_system* sys, const double* R, int k, const double rk[3],
                            double* usum, double grad[3]);
+
+/* ---- kinetic part of the local energy (Alg. 1 L11; definition: lap ln Psi + |grad ln Psi|^2) ---- */
+double oracle_kinetic_energy(const oracle_system* sys, const double* R /*[N][3]*/, const double* B_up /*[n][n]*/,
+                             const double* B_dn, double* e_elec /*[N] or NULL*/);
 
 /* ---- C2/C5/C6: determinants ---- */
 int  oracle_lu_inverse_transpose(int n, const double* A, double* B, double* logabsdet, int* sign);
