@@ -194,6 +194,9 @@ def algorithmic(wl, W, kd, alpha, el, m_move=None):
         "window": {"bytes": W * (kd * (64 * M * el + 8 * n + 3 * M * el)
                                  + alpha * kd * (4 * M * el + 16 * n + 16 * n * (kd - 1) / 2) + 24 * N),
                    "flops": kd * W * 600 * M},
+        # kinetic energy: both inverses, the four cache rows of every electron, positions; ~30 fp64 flop per pair term
+        # (min image, rsqrt, reciprocal, u', u'') and 8 per (electron, orbital) of the four dots
+        "kinetic": {"bytes": W * (16 * n * n + 4 * N * M * el + 24 * N), "flops": W * (30.0 * N * (N - 1) + 8.0 * N * M)},
         "rank1": {"bytes": alpha * W * 16 * n * n, "flops": alpha * W * 4 * n * n},
         "flush": {"bytes": W * 16 * n * n, "flops": W * (4 * n * n * m_flush + 2 * n * m_flush ** 2)},
     }
@@ -305,6 +308,8 @@ def run_cuda(args):
             crowd.qmc_ratio_grad(k)
             crowd.qmc_accept_reject(k)
         crowd.qmc_flush_delayed()
+        crowd.qmc_kinetic_energy()
+        crowd.qmc_kinetic_energy()
         step_prof = {k2: v for k2, v in crowd.profile().items() if v[1] and k2 != "flush"}
     crowd.set_option(q.QMC_OPT_PROFILE, 0)
     tot_ms = sum(v[0] for v in prof.values()) or 1.0
@@ -349,6 +354,14 @@ def run_cuda(args):
             "unit": "TFLOP/s", "frac": useful / pk["fp64_tflops"], "traffic": traffic.get("flush"),
             "peak_source": pk["fp64_source"], "share_of_step": kernels["flush"]["share"],
             "executed_tflops_with_padding": executed, "hbm_frac": kernels["flush"]["hbm_frac"]}
+    if "kinetic" in kernels:
+        # plain fp64 ALU work (J2 pair terms): peak = 148 SMs x 64 FMA/clk x 2 x max SM clock
+        k_ = kernels["kinetic"]
+        tf = alg["kinetic"]["flops"] / (k_["avg_us"] * 1e-6) / 1e12
+        alu_peak = 148 * 64 * 2 * 1.965e9 / 1e12
+        extra_rooflines["kinetic"] = {"kernel": "kinetic_kernel (qmc_kinetic_energy)", "bound": "alu", "achieved": tf,
+                                      "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak, "traffic": None,
+                                      "avg_us": k_["avg_us"], "hbm_frac": k_["hbm_frac"]}
     for name in ("spline_vgl", "rank1"):
         if name in kernels:
             extra_rooflines[name] = {"kernel": name, "bound": "hbm", "achieved": kernels[name]["gbs"],

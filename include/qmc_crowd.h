@@ -130,6 +130,15 @@ int qmc_sweep(qmc_crowd_t* crowd, int n_sweeps);
  * (proposed, accepted, flushes; totals since create) into stats_host[3].  Synchronous.       */
 int qmc_sweep_host(qmc_crowd_t* crowd, double* pos_host, int n_sweeps, uint64_t* stats_host);
 
+/* Kinetic part of the local energy of every walker at its current configuration (Alg. 1 line 11, PAPER.md:59 and
+ * :77 "local energy ... expensive"; the potential part needs pseudopotentials / Ewald sums and
+ * is out of scope):  ekin[w] = -1/2 sum_k lap_k Psi / Psi,  lap_k Psi / Psi = lap_k ln Psi + |grad_k ln Psi|^2,
+ * Psi = D_up D_dn Psi_J, atomic units.  Uses the carried inverses, the per-electron gradient / Laplacian caches and
+ * the positions; changes no state.  ekin_dev: DEVICE [W] fp64 (required); e_elec_dev: DEVICE [W][N] fp64 per-electron
+ * terms or NULL.  Asynchronous on desc.stream.  QMC_ERR_STATE in the middle of a move or with an open delayed window
+ * (call qmc_flush_delayed first; qmc_sweep always returns flushed).                                              */
+int qmc_kinetic_energy(qmc_crowd_t* crowd, double* ekin_dev, double* e_elec_dev);
+
 /* ---- state access for tests: synchronous copies on desc.stream -------------------------- */
 int qmc_crowd_get_positions(qmc_crowd_t* crowd, double* pos_dev /* DEVICE [W][N][3] */);
 int qmc_crowd_set_positions(qmc_crowd_t* crowd, const double* pos_dev); /* rebuilds, may be SINGULAR */
@@ -176,7 +185,8 @@ enum {
   QMC_K_RATIO_ACCEPT = 6,/* qmc_sweep only: ratio_grad + accept of electron k in one kernel      */
   QMC_K_FUSED_MOVE = 7,  /* qmc_sweep only: ratio_grad + accept of k, row/proposal of k+1        */
   QMC_K_WINDOW = 8,      /* qmc_sweep, delay_rank > 1: all moves of one delay window, CTA per walker */
-  QMC_N_KERNEL_CLASSES = 9
+  QMC_K_KINETIC = 9,     /* qmc_kinetic_energy                                                   */
+  QMC_N_KERNEL_CLASSES = 10
 };
 /* Device time (ms, CUDA events on desc.stream) and launch count per kernel class accumulated in
  * profile mode since the previous call; resets the accumulators.  Synchronous.  ms and count

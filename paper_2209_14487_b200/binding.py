@@ -18,11 +18,11 @@ QMC_OPT_GRAPH = 0
 QMC_OPT_PROFILE = 1
 QMC_OPT_SUBCROWDS = 2
 KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush", "ratio_accept",
-                  "fused_move", "window")
+                  "fused_move", "window", "kinetic")
 
 EXPORTS = [
     "qmc_crowd_workspace_bytes", "qmc_crowd_create", "qmc_crowd_destroy", "qmc_spo_vgl", "qmc_ratio_grad",
-    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_crowd_get_positions",
+    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_kinetic_energy", "qmc_crowd_get_positions",
     "qmc_crowd_set_positions", "qmc_crowd_get_inverse", "qmc_crowd_set_inverse", "qmc_crowd_get_caches",
     "qmc_crowd_get_window", "qmc_crowd_get_move", "qmc_crowd_set_sweep_index", "qmc_crowd_stats",
     "qmc_crowd_launch_count", "qmc_crowd_set_option", "qmc_crowd_get_profile", "qmc_last_error", "qmc_version",
@@ -73,6 +73,7 @@ def load():
     L.qmc_flush_delayed.argtypes = [vp]
     L.qmc_sweep.argtypes = [vp, ip]
     L.qmc_sweep_host.argtypes = [vp, vp, ip, vp]
+    L.qmc_kinetic_energy.argtypes = [vp, dp, dp]
     L.qmc_crowd_get_positions.argtypes = [vp, dp]
     L.qmc_crowd_set_positions.argtypes = [vp, dp]
     L.qmc_crowd_get_inverse.argtypes = [vp, ip, dp]
@@ -188,6 +189,15 @@ class Crowd:
         stats = (C.c_uint64 * 3)()
         _check(load().qmc_sweep_host(self._h, pos_host.data_ptr(), n_sweeps, stats))
         return {"proposed": stats[0], "accepted": stats[1], "flushes": stats[2]}
+
+    def qmc_kinetic_energy(self, per_electron=False):
+        """Kinetic energy of every walker, device fp64 [W] (and the per-electron terms [W][N] if asked)."""
+        t = self.torch
+        ekin = t.empty((self.W,), dtype=t.float64, device=self.device)
+        e = t.empty((self.W, self.N), dtype=t.float64, device=self.device) if per_electron else None
+        with t.cuda.stream(self.stream):
+            _check(load().qmc_kinetic_energy(self._h, ekin.data_ptr(), e.data_ptr() if per_electron else None))
+        return (ekin, e) if per_electron else ekin
 
     # -- state access ------------------------------------------------------------------------
     def positions(self):

@@ -41,6 +41,7 @@ struct CrowdDev {
   double *V, *C, *Cp, *Sinv, *pvec, *yvec;
   int* rows;                                 // [W][kdp]
   int* mwin;                                 // [W]
+  double* e_elec;                            // [W][N] per-electron kinetic terms (qmc_kinetic_energy)
   unsigned long long* counters;              // [0] accepted moves
   unsigned* sweep;                           // [1] Philox counter word 2
   int* status;                               // [1] != 0: singular matrix met

@@ -15,6 +15,7 @@
 #include "invert.cuh"
 #include "move.cuh"
 #include "spline.cuh"
+#include "energy.cuh"
 #include "update.cuh"
 #include "window.cuh"
 
@@ -151,6 +152,7 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
   char* yvec = take(W * kdp * 8);
   char* rows = take(W * kdp * 4);
   char* mwin = take(W * 4);
+  char* e_elec = take(W * N * 8);
   char* counters = take(4 * 8);
   char* sweep = take(4);
   char* status = take(4);
@@ -160,6 +162,7 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
     d->usum_old = (double*)usum_old; d->rho_d = (double*)rho_d; d->rho_j = (double*)rho_j;
     d->p = (double*)p; d->u = (double*)u; d->accepted = (unsigned char*)accepted;
     d->V = (double*)V; d->C = (double*)C; d->Cp = (double*)Cp; d->Sinv = (double*)Sinv; d->pvec = (double*)pvec; d->yvec = (double*)yvec;
+    d->e_elec = (double*)e_elec;
     d->rows = (int*)rows; d->mwin = (int*)mwin; d->counters = (unsigned long long*)counters;
     d->sweep = (unsigned*)sweep; d->status = (int*)status;
     (void)acc_sink;
@@ -824,6 +827,31 @@ int qmc_crowd_get_move(qmc_crowd_t* c, double* rnew, double* delta, double* g_ol
     if (st) return st;
   }
   CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return QMC_OK;
+}
+
+int qmc_kinetic_energy(qmc_crowd_t* c, double* ekin_dev, double* e_elec_dev)
+{
+  if (!c || !ekin_dev) return fail(QMC_ERR_INVALID_ARG, "NULL argument");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_kinetic_energy in the middle of a move");
+  if (!c->win_rows.empty()) return fail(QMC_ERR_STATE, "qmc_kinetic_energy needs a flushed window (call qmc_flush_delayed)");
+  const CrowdDev& d = c->dev;
+  const size_t smem = (size_t)(3 * d.N + 32) * 8;
+  dim3 grid((d.N + EKIN_EPB - 1) / EKIN_EPB, d.W);
+  {
+    ProfScope ps(c, QMC_K_KINETIC);
+    if (c->is_f64) {
+      if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(kinetic_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      kinetic_kernel<double><<<grid, EKIN_NT, smem, c->stream>>>(d, d.e_elec);
+    } else {
+      if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(kinetic_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      kinetic_kernel<float><<<grid, EKIN_NT, smem, c->stream>>>(d, d.e_elec);
+    }
+    LAUNCH_CHECK(c);
+    kinetic_sum_kernel<<<(d.W + 3) / 4, 128, 0, c->stream>>>(d.W, d.N, d.e_elec, ekin_dev);
+    LAUNCH_CHECK(c);
+  }
+  if (e_elec_dev) CUDA_TRY(cudaMemcpyAsync(e_elec_dev, d.e_elec, (size_t)d.W * d.N * 8, cudaMemcpyDeviceToDevice, c->stream));
   return QMC_OK;
 }
 
