@@ -444,14 +444,15 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
   }
   // GEMM 2: B_strip = B0_strip + nw Z, 16 columns at a time
   {
+    // chunks in reverse order: the strip lines GEMM 1 read last are the most likely to still be in L2
     Frag2<KB> fa, fb;
-    load_frag2<KB>(fa, a0p, a1p, zp, 0, ns, m, mb, t);
-    for (int j0 = 0; j0 < ns; j0 += 32) {
-      if (j0 + 16 < ns) load_frag2<KB>(fb, a0p, a1p, zp, j0 + 16, ns, m, mb, t);
+    load_frag2<KB>(fa, a0p, a1p, zp, ns - 16, ns, m, mb, t);
+    for (int j0 = ns - 16; j0 >= 0; j0 -= 32) {
+      if (j0 >= 16) load_frag2<KB>(fb, a0p, a1p, zp, j0 - 16, ns, m, mb, t);
       mma_store_frag2<KB>(fa, acc, mb, a0p + j0, a1p + j0);
-      if (j0 + 16 < ns) {
-        if (j0 + 32 < ns) load_frag2<KB>(fa, a0p, a1p, zp, j0 + 32, ns, m, mb, t);
-        mma_store_frag2<KB>(fb, acc, mb, a0p + j0 + 16, a1p + j0 + 16);
+      if (j0 >= 16) {
+        if (j0 >= 32) load_frag2<KB>(fa, a0p, a1p, zp, j0 - 32, ns, m, mb, t);
+        mma_store_frag2<KB>(fb, acc, mb, a0p + j0 - 16, a1p + j0 - 16);
       }
     }
   }
