@@ -428,6 +428,16 @@ int sweep_once(qmc_crowd* c)
     LAUNCH_CHECK(c);
     return QMC_OK;
   }
+  if (d.ns <= SWEEP1_MAX_NS) {
+    // small matrices: the whole sweep in one walker-persistent launch (window.cuh, sweep1_kernel)
+    ProfScope ps(c, QMC_K_WINDOW);
+    if (c->is_f64) sweep1_kernel<double><<<d.W, MOVE_NT, window_smem(d, 8), c->stream>>>(d);
+    else sweep1_kernel<float><<<d.W, MOVE_NT, window_smem(d, 4), c->stream>>>(d);
+    LAUNCH_CHECK(c);
+    bump_sweep_kernel<<<1, 1, 0, c->stream>>>(d.sweep);
+    LAUNCH_CHECK(c);
+    return QMC_OK;
+  }
   {
     ProfScope ps(c, QMC_K_ROW_PROPOSE);
     st = c->is_f64 ? launch_row_propose_t<double>(c, 0, nullptr) : launch_row_propose_t<float>(c, 0, nullptr);
@@ -568,6 +578,9 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
     if (wsm > 48 * 1024) {
       e = c->is_f64 ? cudaFuncSetAttribute(window_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm)
                     : cudaFuncSetAttribute(window_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm);
+      if (e == cudaSuccess)
+        e = c->is_f64 ? cudaFuncSetAttribute(sweep1_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm)
+                      : cudaFuncSetAttribute(sweep1_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm);
       if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
     }
   }

@@ -235,4 +235,125 @@ __global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(Crowd
   if (tid == 0) d.mwin[w] = m;
 }
 
+// ---- qmc_sweep with delay_rank = 1 and small matrices: the whole sweep in one launch -------------------
+// Sherman-Morrison after every accepted move (D:C5) touches the full n x n inverse.  For large n that is the
+// bandwidth-bound rank1_kernel spread over the whole GPU (update.cuh); for ns <= SWEEP1_MAX_NS (configs 1 and
+// 2 of BASELINE.json: n = 4 and 32) a move takes microseconds and four launches per move are pure overhead
+// (P:105), so here a CTA owns a walker for the whole sweep and applies the update itself, row by row, with
+// exactly rank1_kernel's arithmetic (same lane partition, same fma order: bit-identical inverses).
+constexpr int SWEEP1_MAX_NS = 128;
+
+// B'[i,:] = B[i,:] - ((B[i,:].phi' - [i == kk]) / rho_D) b_old for all n rows of one spin block, in place.
+// b_old = b_s and phi' = vgl_s[0..ns) in shared memory; row kk_next also goes to next_s (next move's row).
+template <typename T>
+__device__ __forceinline__ void sm_update_rows(double* B, int ns, int n, int kk, double inv_rho, const T* vgl_s,
+                                               const double* b_s, int kk_next, double* next_s)
+{
+  constexpr int RB = 4, NV = SWEEP1_MAX_NS / 64;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nh = ns / 2;
+  double2 ph[NV], bold[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    const int jj = lane + 32 * v;
+    ph[v] = jj < nh ? ld_x2(vgl_s, jj) : make_double2(0.0, 0.0);
+    bold[v] = jj < nh ? reinterpret_cast<const double2*>(b_s)[jj] : make_double2(0.0, 0.0);
+  }
+  for (int i0 = warp * RB; i0 < n; i0 += MOVE_NW * RB) {
+    double2 x[RB][NV];
+#pragma unroll
+    for (int r = 0; r < RB; ++r)
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const int jj = lane + 32 * v;
+        x[r][v] = (i0 + r < n && jj < nh) ? reinterpret_cast<const double2*>(B + (size_t)(i0 + r) * ns)[jj]
+                                          : make_double2(0.0, 0.0);
+      }
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      const int i = i0 + r;
+      if (i >= n) break;
+      double acc = 0.0;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        acc = fma(x[r][v].x, ph[v].x, acc);
+        acc = fma(x[r][v].y, ph[v].y, acc);
+      }
+      acc = warp_sum(acc);
+      const double f = (acc - (i == kk ? 1.0 : 0.0)) * inv_rho;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const int jj = lane + 32 * v;
+        if (jj < nh) {
+          x[r][v].x = fma(-f, bold[v].x, x[r][v].x);
+          x[r][v].y = fma(-f, bold[v].y, x[r][v].y);
+          reinterpret_cast<double2*>(B + (size_t)i * ns)[jj] = x[r][v];
+          if (i == kk_next) reinterpret_cast<double2*>(next_s)[jj] = x[r][v];
+        }
+      }
+    }
+  }
+}
+
+// dynamic smem: win_layout(...).total doubles (same layout as the window kernel).  ns <= SWEEP1_MAX_NS.
+template <typename T>
+__global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) sweep1_kernel(CrowdDev d)
+{
+  extern __shared__ double sm[];
+  __shared__ SplineW<T> sw;
+  const int w = blockIdx.x + d.w0, ns = d.ns, n = d.n, tid = threadIdx.x;
+  const WinLayout L = win_layout(d.N, ns, d.kdp, (int)sizeof(T));
+  double* R_s = sm + L.R;
+  double* b_s = sm + L.b;
+  double* bn_s = sm + L.bn;
+  double* red = sm + L.red;
+  double* gauss = sm + L.gauss;
+  const int cstride = ((3 * ns * (int)sizeof(T) + 15) / 16) * 16 / (int)sizeof(T);
+  T* cbuf = reinterpret_cast<T*>(sm + L.cbuf);
+  T* vgl_s = reinterpret_cast<T*>(sm + L.vgl);
+  const MoveScal ms = move_scal_smem(sm + L.mv);
+  double* Bw = d.Binv + (size_t)w * 2 * ns * ns;
+  double* Rg = d.R + (size_t)w * d.N * 3;
+  T* cache0 = static_cast<T*>(d.cache) + (size_t)w * d.N * 4 * ns;
+  const int row_bytes = ns * 8, cache_bytes = 3 * ns * (int)sizeof(T);
+
+  cp_async_cta(b_s, Bw, row_bytes);
+  cp_async_cta(cbuf, cache0, cache_bytes);
+  for (int j = tid; j < 3 * d.N; j += MOVE_NT) R_s[j] = Rg[j];
+  if (tid >= 32 && tid < 37) gauss[tid - 32] = gauss_piece(d, w, 0, tid - 32);
+  cp_async_wait_all();
+  __syncthreads();
+
+  for (int k = 0; k < d.N; ++k) {
+    const int spin = k / n, kk = k - spin * n;
+    double* B = Bw + (size_t)spin * ns * ns;
+    T* ccur = cbuf + (k & 1) * cstride;
+    T* cache_g = cache0 + (size_t)k * 4 * ns;
+    const bool more = k + 1 < d.N;
+    const int spin1 = (k + 1) / n, kk1 = (k + 1) - spin1 * n;
+    if (more) {
+      cp_async_cta(bn_s, Bw + ((size_t)spin1 * ns + kk1) * ns, row_bytes);
+      cp_async_cta(cbuf + ((k + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
+    }
+    dev_gold_propose<T>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss, &sw);
+    spline_cta<T, MOVE_NT>(d, nullptr, sw, vgl_s, [&](int t) {
+      if (more && t < 37) gauss[t - 32] = gauss_piece(d, w, k + 1, t - 32);
+    });
+    __syncthreads();
+    dev_ratio_grad<T>(d, w, k, b_s, vgl_s, R_s, ms, nullptr, nullptr, red);
+    cp_async_wait_all();
+    if (dev_decide(d, w, k, ms, nullptr)) {
+      const double inv_rho = 1.0 / *ms.rho_d;
+      for (int j = tid; j < 4 * ns; j += MOVE_NT) cache_g[j] = vgl_s[ns + j];
+      if (tid < 3) {
+        const double x = ms.rn[tid];
+        R_s[3 * k + tid] = x;
+        Rg[3 * k + tid] = x;
+      }
+      sm_update_rows<T>(B, ns, n, kk, inv_rho, vgl_s, b_s, (more && spin1 == spin) ? kk1 : -1, bn_s);
+    }
+    __syncthreads();
+    double* t = b_s; b_s = bn_s; bn_s = t;
+  }
+}
+
 }  // namespace qmc
