@@ -187,12 +187,24 @@ __global__ void __launch_bounds__(INVB_NT) invert_blocked_kernel(CrowdDev d)
       for (int r = tid; r < n; r += INVB_NT) colf[r] = XG[r * INVB_XS + j];
       if (tid < nb) rowc[tid] = (tid == j) ? 1.0 / pv : XG[c * INVB_XS + tid] / pv;   // true divisions (see above)
       __syncthreads();
-      for (int e = tid; e < n * nb; e += INVB_NT) {
-        const int r = e / nb, jj = e - r * nb;
-        double v;
-        if (r == c) v = rowc[jj];
-        else v = fma(-colf[r], rowc[jj], (jj == j) ? 0.0 : XG[r * INVB_XS + jj]);
-        XG[r * INVB_XS + jj] = v;
+      if (nb == INVB_NB) {   // full panel: index arithmetic by shifts (an integer division per element otherwise)
+        static_assert((INVB_NB & (INVB_NB - 1)) == 0 && INVB_NT % INVB_NB == 0, "panel width must be a power of two");
+        const int jj = tid & (INVB_NB - 1);
+        const double rc = rowc[jj];
+        for (int r = tid / INVB_NB; r < n; r += INVB_NT / INVB_NB) {
+          double v;
+          if (r == c) v = rc;
+          else v = fma(-colf[r], rc, (jj == j) ? 0.0 : XG[r * INVB_XS + jj]);
+          XG[r * INVB_XS + jj] = v;
+        }
+      } else {
+        for (int e = tid; e < n * nb; e += INVB_NT) {
+          const int r = e / nb, jj = e - r * nb;
+          double v;
+          if (r == c) v = rowc[jj];
+          else v = fma(-colf[r], rowc[jj], (jj == j) ? 0.0 : XG[r * INVB_XS + jj]);
+          XG[r * INVB_XS + jj] = v;
+        }
       }
       __syncthreads();
     }

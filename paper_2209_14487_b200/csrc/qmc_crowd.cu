@@ -222,7 +222,7 @@ int rebuild(qmc_crowd* c)
   int st = c->is_f64 ? launch_build_t<double>(c) : launch_build_t<float>(c);
   if (st) return st;
   const size_t bsmem = invert_blocked_smem(d.ns);
-  if (bsmem <= 227 * 1024) {
+  if (bsmem <= 227 * 1024 && d.ns <= INVB_NT) {
     if (bsmem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_blocked_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsmem));
     invert_blocked_kernel<<<(unsigned)(d.W * 2), INVB_NT, bsmem, c->stream>>>(d);
   } else {
