@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(RANK1_NT) rank1_generic_kernel(CrowdDev d, int
 #define QMC_FLUSH_PFD1 0
 #endif
 #ifndef QMC_FLUSH_PFD
-#define QMC_FLUSH_PFD 8
+#define QMC_FLUSH_PFD 0
 #endif
 #ifndef QMC_FLUSH_MIN_CTAS
 #define QMC_FLUSH_MIN_CTAS 3
@@ -289,7 +289,10 @@ __global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize
 //  - a K-split form (eight warps share a strip, each keeps its columns in registers, partial products summed through
 //    shared memory, strip read once: 10.3 GB of traffic) ran at 5.0 ms instead of 3.3 ms: two block barriers per strip
 //    and eight warps per SM leave the DMMA pipe 42 % busy;
-//  - 8-row strips (half the L2 reuse distance, twice the V fragment traffic per DMMA): 4.1 ms instead of 3.7 ms.
+//  - 8-row strips (half the L2 reuse distance, twice the V fragment traffic per DMMA): 4.1 ms instead of 3.7 ms;
+//  - a pair of warps per strip splitting its columns (partials exchanged through shared memory, second read half a
+//    strip after the first): 4.4 ms instead of 3.5 ms -- the exposed load latency at the start of each shorter
+//    GEMM loop costs more than the L2 hits save.
 // ---- strip kernel: fragments straight from global memory, software-pipelined in registers -------
 // (A shared-memory cp.async ring for the operands was measured slower on B200 in round 1: 2.54 ms vs 2.07 ms per
 // flush at cfg 5 / W = 2048 -- the LDS + LDGSTS instruction stream saturates the MIO queue next to
@@ -307,7 +310,8 @@ __device__ __forceinline__ void load_frag1(Frag1<KB>& f, const double* a0p, cons
   ld32_keep(a0p + s, f.a0);
   ld32_keep(a1p + s, f.a1);
 #if QMC_FLUSH_PFD > 0
-  // the strip of B0 is the DRAM stream of this kernel: pull its lines into L2 QMC_FLUSH_PFD chunks ahead
+  // optional L2 prefetch of the strip QMC_FLUSH_PFD chunks ahead (off: with GEMM 2 walking the strip in reverse the
+  // prefetch only competes for L2; 3.54 ms without, 3.63 ms with, at cfg 5 / W = 4096)
   if ((threadIdx.x & 3) == 0 && s + 16 * QMC_FLUSH_PFD < ns) {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(a0p + s + 16 * QMC_FLUSH_PFD));
     asm volatile("prefetch.global.L2 [%0];" ::"l"(a1p + s + 16 * QMC_FLUSH_PFD));
