@@ -121,7 +121,11 @@ int qmc_flush_delayed(qmc_crowd_t* crowd);
 
 /* BJ "qmc_sweep": n_sweeps full sweeps k = 0..N-1 (P:73 particle-by-particle; Alg. 3 lines 2-4)
  * of propose / vgl / ratio / accept with the flush schedule of D:C6; the sweep index (Philox
- * counter word 2) advances by one per sweep.  Ends flushed.  Asynchronous.                    */
+ * counter word 2) advances by one per sweep.  Ends flushed.  Asynchronous.
+ * Same moves, decisions and positions as the step calls issued in that order; with delay_rank > 1 the
+ * crowd advances in lock-step per delay window (a walker's moves of a window run back to back, DESIGN.md
+ * R5) and the inverses agree with the step-call path to rounding (1e-10).  Requires the per-walker state
+ * of a move (about 42 KB at N = 768) to fit shared memory: N up to a few thousand.                     */
 int qmc_sweep(qmc_crowd_t* crowd, int n_sweeps);
 
 /* Host-buffer form of the same path (bench.py "e2e"): copies pos_host (HOST, [W][N][3] fp64)
@@ -182,9 +186,9 @@ enum {
   QMC_K_ACCEPT = 3,      /* Metropolis decision, cache update, window append (steps a3, a4')     */
   QMC_K_RANK1 = 4,       /* Sherman-Morrison rank-1 update (step a4)                             */
   QMC_K_FLUSH = 5,       /* delayed rank-k flush, FP64 DMMA (step a5)                            */
-  QMC_K_RATIO_ACCEPT = 6,/* qmc_sweep only: ratio_grad + accept of electron k in one kernel      */
-  QMC_K_FUSED_MOVE = 7,  /* qmc_sweep only: ratio_grad + accept of k, row/proposal of k+1        */
-  QMC_K_WINDOW = 8,      /* qmc_sweep, delay_rank > 1: all moves of one delay window, CTA per walker */
+  QMC_K_RATIO_ACCEPT = 6,/* qmc_sweep, delay_rank 1, large n: ratio_grad + accept of electron k  */
+  QMC_K_FUSED_MOVE = 7,  /* (no longer launched; kept so that class numbers stay stable)         */
+  QMC_K_WINDOW = 8,      /* qmc_sweep: all moves of one delay window (or, delay_rank 1 and small n, of a sweep), CTA per walker */
   QMC_K_KINETIC = 9,     /* qmc_kinetic_energy                                                   */
   QMC_N_KERNEL_CLASSES = 10
 };
