@@ -51,16 +51,6 @@ template <typename T> struct Vec16;
 template <> struct Vec16<float> { static constexpr int W = 4; };
 template <> struct Vec16<double> { static constexpr int W = 2; };
 
-__device__ __forceinline__ void ld16(const float* p, float (&v)[4])
-{
-  const float4 q = __ldg(reinterpret_cast<const float4*>(p));
-  v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
-}
-__device__ __forceinline__ void ld16(const double* p, double (&v)[2])
-{
-  const double2 q = __ldg(reinterpret_cast<const double2*>(p));
-  v[0] = q.x; v[1] = q.y;
-}
 // Streaming 16-byte loads of read-only data with an L2 evict-first policy (the spline table is gathered once per
 // move and must not push the per-walker state out of L2: window kernel 4.94 -> 4.63 ms at cfg 5, W = 4096; an
 // evict_last policy on the walker's own block rows, tried on top, was slightly slower and is not used).

@@ -15,10 +15,6 @@
 #pragma once
 #include "common.cuh"
 
-#ifndef QMC_SPLINE_STREAM
-#define QMC_SPLINE_STREAM 1
-#endif
-
 namespace qmc {
 
 // Per-position weights, built once per evaluation in shared memory.
@@ -79,18 +75,12 @@ __device__ __forceinline__ void spline_plane_load(const T* __restrict__ tab, con
 {
   constexpr int VW = Vec16<T>::W;
   const unsigned base = s.off[0][a] + chunk;
-#if QMC_SPLINE_STREAM
-  const unsigned long long pol = l2_evict_first_policy();
-#endif
+  const unsigned long long pol = l2_evict_first_policy();   // streaming gather: see ld16_stream
 #pragma unroll
   for (int b = 0; b < 4; ++b)
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
-#if QMC_SPLINE_STREAM
       ld16_stream(tab + (size_t)(base + s.off[1][b] + s.off[2][c]) * VW, p[b][c], pol);
-#else
-      ld16(tab + (size_t)(base + s.off[1][b] + s.off[2][c]) * VW, p[b][c]);
-#endif
     }
 }
 

@@ -102,12 +102,6 @@ __global__ void __launch_bounds__(RANK1_NT) rank1_generic_kernel(CrowdDev d, int
   }
 }
 
-#ifndef QMC_FLUSH_PFD1
-#define QMC_FLUSH_PFD1 0
-#endif
-#ifndef QMC_FLUSH_PFD
-#define QMC_FLUSH_PFD 0
-#endif
 #ifndef QMC_FLUSH_MIN_CTAS
 #define QMC_FLUSH_MIN_CTAS 3
 #endif
@@ -124,37 +118,9 @@ __device__ __forceinline__ void ld32(const double* p, double (&v)[4])
 {
   asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
 }
-// The strip of B0 is read twice (GEMM 1 operand, GEMM 2 accumulator) and written once: the first read asks L2 to
-// keep the lines (evict_last), the second read and the store mark them as dead (evict_first), so the strips in flight
-// (148 SMs x 12 warps x 48 KB) survive between the two passes instead of being pushed out by the streaming stores.
-// Measured on B200 (cfg 5, W = 4096): no change in kernel time (3.67 vs 3.66 ms per flush), so it is off by default.
-#ifndef QMC_FLUSH_L2HINT
-#define QMC_FLUSH_L2HINT 0
-#endif
-__device__ __forceinline__ void ld32_keep(const double* p, double (&v)[4])
-{
-#if QMC_FLUSH_L2HINT
-  asm volatile("ld.global.L2::evict_last.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
-#else
-  ld32(p, v);
-#endif
-}
-__device__ __forceinline__ void ld32_last(const double* p, double (&v)[4])
-{
-#if QMC_FLUSH_L2HINT
-  asm volatile("ld.global.L1::no_allocate.L2::evict_first.v4.f64 {%0,%1,%2,%3}, [%4];"
-               : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
-#else
-  ld32(p, v);
-#endif
-}
 __device__ __forceinline__ void st32(double* p, double a, double b, double c, double d)
 {
-#if QMC_FLUSH_L2HINT
-  asm volatile("st.global.L2::evict_first.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-#else
   asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-#endif
 }
 
 // Flush, step 1 (per walker, column-local): Z = S^-T C, Z[l][j] = sum_q Sinv[q][l] C[q][j], written to
@@ -284,8 +250,9 @@ __global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize
 //    fragments loaded straight from L1/L2 as here -- the operand path is not the limit, DRAM streaming is: the strip is
 //    read twice and the second read misses L2 half the time (13.8 GB of traffic for 9.7 GB algorithmic; skipping the
 //    second read shortens the flush by 0.85 ms);
-//  - L2 eviction hints (QMC_FLUSH_L2HINT) with or without a persisting-L2 set-aside: no gain (the set-aside slows the
-//    window kernel);
+//  - L2 eviction hints on the strip (evict_last on the first read, evict_first on the second read and the store) with
+//    or without a persisting-L2 set-aside, and L2 / L1 prefetches of the strip 2-16 chunks ahead: no gain (the
+//    set-aside slows the window kernel; with GEMM 2 walking backwards the L2 prefetch costs 0.1 ms);
 //  - a K-split form (eight warps share a strip, each keeps its columns in registers, partial products summed through
 //    shared memory, strip read once: 10.3 GB of traffic) ran at 5.0 ms instead of 3.3 ms: two block barriers per strip
 //    and eight warps per SM leave the DMMA pipe 42 % busy;
@@ -307,22 +274,8 @@ template <int KB>
 __device__ __forceinline__ void load_frag1(Frag1<KB>& f, const double* a0p, const double* a1p, const double* vp,
                                            int s, int ns, int m, int mb, int g)
 {
-  ld32_keep(a0p + s, f.a0);
-  ld32_keep(a1p + s, f.a1);
-#if QMC_FLUSH_PFD > 0
-  // optional L2 prefetch of the strip QMC_FLUSH_PFD chunks ahead (off: with GEMM 2 walking the strip in reverse the
-  // prefetch only competes for L2; 3.54 ms without, 3.63 ms with, at cfg 5 / W = 4096)
-  if ((threadIdx.x & 3) == 0 && s + 16 * QMC_FLUSH_PFD < ns) {
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(a0p + s + 16 * QMC_FLUSH_PFD));
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(a1p + s + 16 * QMC_FLUSH_PFD));
-  }
-#endif
-#if QMC_FLUSH_PFD1 > 0
-  if ((threadIdx.x & 3) == 0 && s + 16 * QMC_FLUSH_PFD1 < ns) {
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(a0p + s + 16 * QMC_FLUSH_PFD1));
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(a1p + s + 16 * QMC_FLUSH_PFD1));
-  }
-#endif
+  ld32(a0p + s, f.a0);
+  ld32(a1p + s, f.a1);
 #pragma unroll
   for (int b = 0; b < KB; ++b) {
     f.v[b][0] = f.v[b][1] = f.v[b][2] = f.v[b][3] = 0.0;
@@ -353,8 +306,8 @@ template <int KB>
 __device__ __forceinline__ void load_frag2(Frag2<KB>& f, const double* a0p, const double* a1p, const double* zp,
                                            int j0, int ns, int m, int mb, int t)
 {
-  ld32_last(a0p + j0, f.x0);
-  ld32_last(a1p + j0, f.x1);
+  ld32(a0p + j0, f.x0);
+  ld32(a1p + j0, f.x1);
 #pragma unroll
   for (int b = 0; b < KB; ++b)
 #pragma unroll
