@@ -3,6 +3,9 @@
 // append (SURVEY 8(a) steps a0, a2, a3, a4').  One CTA of MOVE_NT threads per walker; all
 // length-n / length-N sums are strided over the block and combined by shuffle reductions (BJ).
 //
+// The window kernel instantiates the shared blocks with NT = 128, 256 or 512 threads per walker (small crowds get
+// wider CTAs, window.cuh); the step kernels use MOVE_NT.  Block sums depend on NT at the rounding level only.
+//
 // The building blocks below (row dots, axpy over window rows, the G_k(R)/proposal tail, ratio, decision)
 // are shared by the three step kernels of the C ABI and by the walker-persistent window kernel of
 // qmc_sweep (window.cuh), which is what makes the two paths bit-identical: same products, same
@@ -68,10 +71,11 @@ __device__ __forceinline__ void j2_pair(const CrowdDev& d, const double (&rk)[3]
 }
 
 // Thread-strided partial J2 sums of electron k at rk against all other electrons of R [N][3].
+template <int NT = MOVE_NT>
 __device__ __forceinline__ void j2_partial(const CrowdDev& d, const double* R, int k, const double (&rk)[3], double& usum,
                                            double (&g)[3])
 {
-  for (int i = threadIdx.x; i < d.N; i += MOVE_NT)
+  for (int i = threadIdx.x; i < d.N; i += NT)
     if (i != k) j2_pair(d, rk, R + 3 * i, usum, g);
 }
 
@@ -161,7 +165,7 @@ __device__ __forceinline__ double gauss_piece(const CrowdDev& d, int w, int k, i
 // electron k; R: positions [N][3] of the walker.  The five transcendental pieces of the Gaussians
 // run on five threads (or arrive precomputed in gauss_pre[5]).  Threads 0..2 take one component each, write the
 // results to ms and, if sw_out is given, the spline weights of their axis at r'; callers synchronise before reading.
-template <typename T>
+template <typename T, int NT = MOVE_NT>
 __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k, const double* b_s, const T* cache,
                                                  const double* R, const double* rnew_given, MoveScal ms, double* red,
                                                  const double* gauss_pre = nullptr, SplineW<T>* sw_out = nullptr)
@@ -169,7 +173,7 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
   const int ns = d.ns, tid = threadIdx.x;
   // v[0..2] = b . grad phi(r_k), v[3] = usum_old, v[4..6] = grad_k ln Psi_J(R)
   double v[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-  for (int j = tid; j < d.M; j += MOVE_NT) {
+  for (int j = tid; j < d.M; j += NT) {
     const double bj = b_s[j];
     v[0] = fma(bj, (double)cache[j], v[0]);
     v[1] = fma(bj, (double)cache[ns + j], v[1]);
@@ -178,10 +182,10 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
   const double rk[3] = {R[3 * k], R[3 * k + 1], R[3 * k + 2]};
   {
     double g[3] = {0.0, 0.0, 0.0};
-    j2_partial(d, R, k, rk, v[3], g);
+    j2_partial<NT>(d, R, k, rk, v[3], g);
     v[4] = g[0]; v[5] = g[1]; v[6] = g[2];
   }
-  block_sum_t0<7, MOVE_NT>(v, red);
+  block_sum_t0<7, NT>(v, red);
   if (!rnew_given && !gauss_pre) {
     if (tid < 5) red[tid] = gauss_piece(d, w, k, tid);
     __syncthreads();
@@ -212,14 +216,14 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
 // ---- qmc_ratio_grad ------------------------------------------------------------------------
 // rho_D = b . phi(r'); grad = (b . grad phi(r'))/rho_D + grad_k ln Psi_J(R'); rho_J (D:C2, C3)
 // b: inverse row (window applied); vgl: [5][ns] at r'; R: positions; red: MOVE_RED doubles.
-template <typename T>
+template <typename T, int NT = MOVE_NT>
 __device__ __forceinline__ void dev_ratio_grad(const CrowdDev& d, int w, int k, const double* b, const T* vgl,
                                                const double* R, MoveScal ms, double* ratio_out, double* grad_out,
                                                double* red)
 {
   const int ns = d.ns, tid = threadIdx.x;
   double v[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-  for (int j = tid; j < d.M; j += MOVE_NT) {
+  for (int j = tid; j < d.M; j += NT) {
     const double bj = b[j];
     v[0] = fma(bj, (double)vgl[j], v[0]);
     v[1] = fma(bj, (double)vgl[ns + j], v[1]);
@@ -229,10 +233,10 @@ __device__ __forceinline__ void dev_ratio_grad(const CrowdDev& d, int w, int k, 
   const double rn[3] = {ms.rn[0], ms.rn[1], ms.rn[2]};
   {
     double g[3] = {0.0, 0.0, 0.0};
-    j2_partial(d, R, k, rn, v[4], g);
+    j2_partial<NT>(d, R, k, rn, v[4], g);
     v[5] = g[0]; v[6] = g[1]; v[7] = g[2];
   }
-  block_sum_t0<8, MOVE_NT>(v, red);
+  block_sum_t0<8, NT>(v, red);
   if (tid == 0) {
     const double rho_d = v[0];
     const double rho_j = exp(v[4] - *ms.usum_old);

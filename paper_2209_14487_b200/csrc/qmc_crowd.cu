@@ -376,7 +376,10 @@ int launch_ratio_accept_t(qmc_crowd* c, int k)
   return QMC_OK;
 }
 
-size_t window_smem(const CrowdDev& d, size_t elem) { return (size_t)win_layout(d.N, d.ns, d.kdp, (int)elem).total * 8; }
+size_t window_smem(const CrowdDev& d, size_t elem, int nt = MOVE_NT) { return (size_t)win_layout(d.N, d.ns, d.kdp, (int)elem, nt).total * 8; }
+
+// Threads per walker of the window kernel: a crowd that leaves SMs idle gets wider CTAs (shorter move chain).
+int window_threads(int wn) { return wn <= 148 ? 512 : (wn <= 296 ? 256 : 128); }
 
 template <typename T>
 int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t st)
@@ -384,9 +387,26 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   ProfScope ps(c, QMC_K_WINDOW);
   CrowdDev d = c->dev;
   d.w0 = w0;
-  window_kernel<T><<<wn, MOVE_NT, window_smem(d, sizeof(T)), st>>>(d, k0, cnt);
+  switch (window_threads(wn)) {
+    case 512: window_kernel<T, 512><<<wn, 512, window_smem(d, sizeof(T), 512), st>>>(d, k0, cnt); break;
+    case 256: window_kernel<T, 256><<<wn, 256, window_smem(d, sizeof(T), 256), st>>>(d, k0, cnt); break;
+    default: window_kernel<T, 128><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt); break;
+  }
   LAUNCH_CHECK(c);
   return QMC_OK;
+}
+
+template <typename T>
+cudaError_t window_smem_attr(const CrowdDev& d)
+{
+  cudaError_t e = cudaSuccess;
+  const int s128 = (int)window_smem(d, sizeof(T), 128), s256 = (int)window_smem(d, sizeof(T), 256),
+            s512 = (int)window_smem(d, sizeof(T), 512);
+  if (s128 > 48 * 1024) e = cudaFuncSetAttribute(window_kernel<T, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128);
+  if (e == cudaSuccess && s256 > 48 * 1024) e = cudaFuncSetAttribute(window_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, s256);
+  if (e == cudaSuccess && s512 > 48 * 1024) e = cudaFuncSetAttribute(window_kernel<T, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, s512);
+  if (e == cudaSuccess && s128 > 48 * 1024) e = cudaFuncSetAttribute(sweep1_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128);
+  return e;
 }
 
 // One full sweep with the D:C6 flush schedule; no host synchronisation (capturable).
@@ -563,7 +583,7 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   if (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess)
     return bail(fail(QMC_ERR_CUDA, "sub-crowd event: %s", cudaGetErrorString(cudaGetLastError())));
   {
-    const int sm = (int)move_smem(d), wsm = (int)window_smem(d, c->elem);
+    const int sm = (int)move_smem(d), wsm = (int)window_smem(d, c->elem, 512);
     if (wsm > 227 * 1024 || sm > 227 * 1024)
       return bail(fail(QMC_ERR_INVALID_ARG, "n_elec / delay_rank too large: the per-walker state (%d bytes) exceeds shared memory", wsm));
     const void* fns[] = {(const void*)row_propose_kernel<float>, (const void*)row_propose_kernel<double>,
@@ -575,14 +595,8 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
       e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
       if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
     }
-    if (wsm > 48 * 1024) {
-      e = c->is_f64 ? cudaFuncSetAttribute(window_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm)
-                    : cudaFuncSetAttribute(window_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm);
-      if (e == cudaSuccess)
-        e = c->is_f64 ? cudaFuncSetAttribute(sweep1_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm)
-                      : cudaFuncSetAttribute(sweep1_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, wsm);
-      if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
-    }
+    e = c->is_f64 ? window_smem_attr<double>(d) : window_smem_attr<float>(d);
+    if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
   }
   st = rebuild(c);
   if (st) return bail(st);

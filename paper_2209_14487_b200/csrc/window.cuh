@@ -26,22 +26,19 @@
 
 namespace qmc {
 
-#ifndef QMC_WIN_MIN_CTAS
-#define QMC_WIN_MIN_CTAS (512 / QMC_MOVE_NT)
-#endif
 
 // Shared-memory layout of the window kernel, offsets in doubles.
 struct WinLayout {
   int R, b, bn, red, mv, gauss, rows, cbuf, vgl, total;
 };
-__host__ __device__ inline WinLayout win_layout(int N, int ns, int kdp, int elem)
+__host__ __device__ inline WinLayout win_layout(int N, int ns, int kdp, int elem, int nt = MOVE_NT)
 {
   WinLayout L;
   int o = 0;
   L.R = o; o += 3 * N;       // positions of the walker
   L.b = o; o += ns;          // inverse row of the current move (then c_l = b / rho_D)
   L.bn = o; o += ns;         // inverse row of the next move
-  L.red = o; o += MOVE_RED;
+  L.red = o; o += (8 * (nt / 32) < 32 ? 32 : 8 * (nt / 32));
   L.mv = o; o += MOVE_MV;
   L.gauss = o; o += 8;       // Box-Muller pieces of the next move
   L.rows = o; o += kdp / 2;  // int[kdp]: electron (within the spin block) of accepted move l
@@ -68,9 +65,10 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // nbytes % 16 == 0, both 16-byte aligned; strided over the CTA
+template <int NT = MOVE_NT>
 __device__ __forceinline__ void cp_async_cta(void* smem, const void* gmem, int nbytes)
 {
-  for (int o = threadIdx.x * 16; o < nbytes; o += MOVE_NT * 16)
+  for (int o = threadIdx.x * 16; o < nbytes; o += NT * 16)
     cp_async16(static_cast<char*>(smem) + o, static_cast<const char*>(gmem) + o);
 }
 
@@ -80,7 +78,7 @@ __device__ __forceinline__ void cp_async_cta(void* smem, const void* gmem, int n
 // dot and the update (rows of up to 64 WIN_NV = 512 columns; longer rows are read twice), and also
 // hands row r_first to shared memory (next_s) as the next move's inverse row.
 constexpr int WIN_NV = 8;
-template <typename T>
+template <typename T, int NT>
 __device__ __forceinline__ void block_rows_update(const double* src, double* dst, int ns, int r_first, int cnt,
                                                   const T* vgl_s, const double* c_s, double* next_s)
 {
@@ -88,7 +86,7 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nh = ns / 2;
   const double2* c2 = reinterpret_cast<const double2*>(c_s);
   if (nh <= 32 * WIN_NV) {
-    for (int r0 = r_first + warp * RB; r0 < cnt; r0 += MOVE_NW * RB) {
+    for (int r0 = r_first + warp * RB; r0 < cnt; r0 += (NT / 32) * RB) {
       double2 v[RB][WIN_NV];
       double acc[RB];
 #pragma unroll
@@ -131,7 +129,7 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
       }
     }
   } else {
-    for (int r = r_first + warp; r < cnt; r += MOVE_NW) {
+    for (int r = r_first + warp; r < cnt; r += NT / 32) {
       const double2* rp = reinterpret_cast<const double2*>(src + (size_t)r * ns);
       double2* wp = reinterpret_cast<double2*>(dst + (size_t)r * ns);
       double acc = 0.0;
@@ -152,13 +150,15 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
 
 // dynamic smem: win_layout(...).total doubles.  Requires an empty window on entry (qmc_sweep flushes first).
 // Leaves for the flush: V[l] = phi_l, Cp[l] = c_l, rows[l], mwin (and Bcur in the d.C buffer, dead afterwards).
-template <typename T>
-__global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(CrowdDev d, int k0, int cnt)
+// NT threads per walker: 128 for full crowds (4 CTAs/SM), 256 / 512 when the crowd leaves SMs idle (a move is then a
+// latency chain and wider CTAs shorten every phase of it: +10 % at W = 256, +35 % at W = 64 on cfg 5).
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) window_kernel(CrowdDev d, int k0, int cnt)
 {
   extern __shared__ double sm[];
   __shared__ SplineW<T> sw;
   const int w = blockIdx.x + d.w0, ns = d.ns, kdp = d.kdp, tid = threadIdx.x;
-  const WinLayout L = win_layout(d.N, ns, kdp, (int)sizeof(T));
+  const WinLayout L = win_layout(d.N, ns, kdp, (int)sizeof(T), NT);
   double* R_s = sm + L.R;
   double* b_s = sm + L.b;    // row of the current move
   double* bn_s = sm + L.bn;  // row of the next move
@@ -181,11 +181,11 @@ __global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(Crowd
 
   // prologue: row and gradient cache of the first move, positions, Gaussians of the first move;
   // the rest of the block is pulled into L2 (first-touch DRAM lines the first accepted move reads)
-  cp_async_cta(b_s, blk, row_bytes);
-  cp_async_cta(cbuf, cache0, cache_bytes);
-  for (int j = tid; j < 3 * d.N; j += MOVE_NT) R_s[j] = Rg[j];
+  cp_async_cta<NT>(b_s, blk, row_bytes);
+  cp_async_cta<NT>(cbuf, cache0, cache_bytes);
+  for (int j = tid; j < 3 * d.N; j += NT) R_s[j] = Rg[j];
   if (tid >= 32 && tid < 37) gauss[tid - 32] = gauss_piece(d, w, k0, tid - 32);
-  for (int j = tid; j < (cnt - 1) * row_bytes / 128; j += MOVE_NT)
+  for (int j = tid; j < (cnt - 1) * row_bytes / 128; j += NT)
     asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
   cp_async_wait_all();
   __syncthreads();
@@ -197,26 +197,26 @@ __global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(Crowd
     T* cache_g = cache0 + (size_t)i * 4 * ns;
     const bool more = i + 1 < cnt;
     if (more) {  // next move's row (valid unless this move is accepted, which rewrites it) and gradient cache
-      cp_async_cta(bn_s, (m ? Bcur : blk) + (size_t)(i + 1) * ns, row_bytes);
-      cp_async_cta(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
+      cp_async_cta<NT>(bn_s, (m ? Bcur : blk) + (size_t)(i + 1) * ns, row_bytes);
+      cp_async_cta<NT>(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
     }
     // ---- G_k(R), proposal, orbitals at r' (the next move's Gaussians ride along), ratio, decision ----
-    dev_gold_propose<T>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss, &sw);
-    spline_cta<T, MOVE_NT>(d, nullptr, sw, vgl_s, [&](int t) {
+    dev_gold_propose<T, NT>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss, &sw);
+    spline_cta<T, NT>(d, nullptr, sw, vgl_s, [&](int t) {
       if (more && t < 37) gauss[t - 32] = gauss_piece(d, w, k + 1, t - 32);
     });
     __syncthreads();
-    dev_ratio_grad<T>(d, w, k, b_s, vgl_s, R_s, ms, nullptr, nullptr, red);
+    dev_ratio_grad<T, NT>(d, w, k, b_s, vgl_s, R_s, ms, nullptr, nullptr, red);
     cp_async_wait_all();
     if (dev_decide(d, w, k, ms, nullptr)) {
       const double inv_rho = 1.0 / *ms.rho_d;
-      for (int j = tid; j < ns; j += MOVE_NT) {
+      for (int j = tid; j < ns; j += NT) {
         const double c = b_s[j] * inv_rho;
         b_s[j] = c;
         Cp[(size_t)m * ns + j] = c;
         V[(size_t)m * ns + j] = (double)vgl_s[j];
       }
-      for (int j = tid; j < 4 * ns; j += MOVE_NT) cache_g[j] = vgl_s[ns + j];
+      for (int j = tid; j < 4 * ns; j += NT) cache_g[j] = vgl_s[ns + j];
       if (tid < 3) {
         const double x = ms.rn[tid];
         R_s[3 * k + tid] = x;
@@ -224,14 +224,14 @@ __global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) window_kernel(Crowd
       }
       if (tid == 0) rows_s[m] = kk0 + i;
       __syncthreads();
-      block_rows_update<T>(m ? Bcur : blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
+      block_rows_update<T, NT>(m ? Bcur : blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
       ++m;
     }
     __syncthreads();
     double* t = b_s; b_s = bn_s; bn_s = t;
   }
 
-  for (int l = tid; l < m; l += MOVE_NT) d.rows[(size_t)w * kdp + l] = rows_s[l];
+  for (int l = tid; l < m; l += NT) d.rows[(size_t)w * kdp + l] = rows_s[l];
   if (tid == 0) d.mwin[w] = m;
 }
 
@@ -296,7 +296,7 @@ __device__ __forceinline__ void sm_update_rows(double* B, int ns, int n, int kk,
 
 // dynamic smem: win_layout(...).total doubles (same layout as the window kernel).  ns <= SWEEP1_MAX_NS.
 template <typename T>
-__global__ void __launch_bounds__(MOVE_NT, QMC_WIN_MIN_CTAS) sweep1_kernel(CrowdDev d)
+__global__ void __launch_bounds__(MOVE_NT, 512 / MOVE_NT) sweep1_kernel(CrowdDev d)
 {
   extern __shared__ double sm[];
   __shared__ SplineW<T> sw;
