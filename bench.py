@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--sub-crowds", type=int, default=None, help="sub-crowds qmc_sweep runs on separate streams (1..4)")
+    ap.add_argument("--multi-crowd", action="store_true",
+                    help="also time C crowds of W/C walkers, one stream and one host thread each (PAPER.md Alg. 4)")
     ap.add_argument("--no-probes", action="store_true", help="skip the step-call / rank-1 kernel probes")
     ap.add_argument("--ref-walkers", type=int, default=None, help="walkers of the oracle sample (default = cores)")
     return ap.parse_args()
@@ -230,6 +232,56 @@ def time_sweeps(crowd, steps, warmup, sync_all):
     sync_all()
     s1 = crowd.stats()
     return e0.elapsed_time(e1), s1["proposed"] - s0["proposed"], s1["accepted"] - s0["accepted"], crowd.launch_count() - l0
+
+
+def time_multi_crowd(wl, W, C, kd, coefs_dev, dev, steps=2, warmup=1):
+    """C crowds of W/C walkers (global walker ids), each on its own stream, each driven by its own host thread
+    (Alg. 4).  Device time: a start event on the current stream that every crowd's stream
+    waits for, an end event that waits for every crowd's last launch.  Returns (ms, proposed, accepted)."""
+    import threading
+    import torch
+    wc = W // C
+    streams = [torch.cuda.Stream(device=dev) for _ in range(C)]
+    crowds = []
+    for c in range(C):
+        pos = qi.make_positions(wl, (c + 1) * wc)[c * wc:]
+        import paper_2209_14487_b200 as q
+        crowds.append(q.Crowd(coefs_dev, wl.box, torch.from_numpy(np.ascontiguousarray(pos)).to(dev), tau=wl.tau,
+                              delay_rank=kd, j2_a=wl.j2_a, j2_b=wl.j2_b, seed=wl.seed, walker_id0=c * wc,
+                              stream=streams[c]))
+
+    def drive(n):
+        def one(cr):
+            torch.cuda.set_device(dev)
+            for _ in range(n):
+                cr.qmc_sweep(1)
+        th = [threading.Thread(target=one, args=(cr,)) for cr in crowds]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+
+    drive(warmup)
+    torch.cuda.synchronize()
+    s0 = [cr.stats() for cr in crowds]
+    main = torch.cuda.current_stream(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(main)
+    for st in streams:
+        st.wait_event(e0)
+    drive(steps)
+    for st in streams:
+        main.wait_stream(st)
+    e1.record(main)
+    torch.cuda.synchronize()
+    s1 = [cr.stats() for cr in crowds]
+    prop = sum(b["proposed"] - a["proposed"] for a, b in zip(s0, s1))
+    acc = sum(b["accepted"] - a["accepted"] for a, b in zip(s0, s1))
+    for cr in crowds:
+        cr.close()
+    del crowds
+    torch.cuda.empty_cache()
+    return e0.elapsed_time(e1), prop, acc
 
 
 def ncu_traffic(cfg, W, kd):
@@ -454,6 +506,14 @@ def run_cuda(args):
                 c2.close()
                 del c2
                 torch.cuda.empty_cache()
+    if args.multi_crowd and world == 1:
+        # S:8(f) item 1: does splitting a crowd of W into C crowds on C streams / host threads pay at small W?
+        for W2 in (256, 512, 1024, 4096):
+            for C in (1, 2, 4, 8):
+                ms2, prop2, acc2 = time_multi_crowd(wl, W2, C, kd, coefs_dev, dev)
+                print(json.dumps({"multi_crowd": True, "walkers": W2, "crowds": C, "delay_rank": kd,
+                                  "value": prop2 / (ms2 * 1e-3), "unit": UNIT, "accept_fraction": acc2 / prop2,
+                                  "ms_per_sweep": ms2 / 2}), flush=True)
     return 0
 
 

@@ -192,3 +192,46 @@ def test_sub_crowds_on_separate_streams_do_not_change_results():
         for spin in (0, 1):
             assert np.array_equal(npy(c.inverse(spin)), npy(ref.inverse(spin)))
         assert c.stats() == ref.stats()
+
+
+def test_crowds_on_host_threads_and_streams_equal_one_crowd():
+    """PAPER.md Alg. 4: several crowds, each advanced by its own host thread on its own stream.
+    With global walker ids the union of the crowds is the one big crowd, walker by walker (same threads-per-walker
+    class here, so bit-identical)."""
+    import threading
+    import torch
+    import paper_2209_14487_b200 as q
+    wl = qi.small_workload(n_elec=48, grid=10, box=6.0, coef_dtype="f32", coef_dist="normal", n_walkers=12, tau=0.02,
+                           delay_rank=8, cfg=16)
+    ref, _, coefs, pos = make_pair(wl)
+    ref.qmc_sweep(3)
+    dev = torch.device("cuda:0")
+    tab = torch.from_numpy(coefs).to(dev)
+    parts = [(0, 5), (5, 9), (9, 12)]
+    crowds = []
+    for lo, hi in parts:
+        st = torch.cuda.Stream(device=dev)
+        crowds.append(q.Crowd(tab, wl.box, torch.from_numpy(pos[lo:hi].copy()).to(dev), tau=wl.tau, delay_rank=8,
+                              j2_a=wl.j2_a, j2_b=wl.j2_b, seed=wl.seed, walker_id0=lo, stream=st))
+
+    def drive(c):
+        torch.cuda.set_device(dev)
+        for _ in range(3):
+            c.qmc_sweep(1)
+
+    th = [threading.Thread(target=drive, args=(c,)) for c in crowds]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    torch.cuda.synchronize()
+    Rref = npy(ref.positions())
+    tot = {"proposed": 0, "accepted": 0}
+    for (lo, hi), c in zip(parts, crowds):
+        assert np.array_equal(npy(c.positions()), Rref[lo:hi])
+        for spin in (0, 1):
+            assert np.array_equal(npy(c.inverse(spin)), npy(ref.inverse(spin))[lo:hi])
+        s = c.stats()
+        tot["proposed"] += s["proposed"]
+        tot["accepted"] += s["accepted"]
+    assert tot["proposed"] == ref.stats()["proposed"] and tot["accepted"] == ref.stats()["accepted"]
