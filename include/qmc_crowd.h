@@ -173,7 +173,8 @@ int qmc_crowd_set_option(qmc_crowd_t* crowd, int option, int value);
  * event pair around every kernel (measurement aid for bench.py's roofline; adds event overhead,
  * so throughput numbers are never taken in this mode).                                        */
 #define QMC_OPT_PROFILE 1
-/* option 2 (QMC_OPT_SUBCROWDS): number of sub-crowds (1..4, default 1) qmc_sweep advances on separate internal
+/* option 2 (QMC_OPT_SUBCROWDS): number of sub-crowds (1..4; 0 = automatic, the default: 2 for crowds of one to four
+ * waves of window CTAs, else 1) qmc_sweep advances on separate internal
  * streams when delay_rank > 1 (crowds on independent streams overlap); walkers are independent, so
  * results do not depend on it.  The sub-crowds are forked from and joined back into desc.stream every sweep.    */
 #define QMC_OPT_SUBCROWDS 2

@@ -67,7 +67,8 @@ struct qmc_crowd {
   uint64_t proposed, flushes, launches;
   uint32_t sweep_host;
   int use_graph;
-  int n_sub;                        // sub-crowds of qmc_sweep (delay_rank > 1), each on its own stream
+  int n_sub;                        // sub-crowds of qmc_sweep (delay_rank > 1), each on its own stream; 0 = automatic
+  int n_sm;                         // SMs of the device (sizes the automatic sub-crowd choice)
   cudaStream_t sub_stream[4];
   cudaEvent_t ev_fork, ev_join[4];
   uint64_t graph_launches, graph_flushes;  // per replay of the captured sweep
@@ -421,7 +422,12 @@ int sweep_once(qmc_crowd* c)
     // Walkers never interact, so the crowd may advance as independent sub-crowds (the paper's crowds on separate
     // streams, Alg. 4 / P:135): with two of them the DMMA-bound flush of one overlaps the window kernel of the other.
     // Each sub-crowd is in lock-step with itself; results do not depend on the split (same walkers, same counters).
-    const int nsub = (c->n_sub > 1 && !c->profile && d.W >= 2 * c->n_sub) ? c->n_sub : 1;
+    // Automatic choice (measured): two sub-crowds pay when the crowd is 1-4 waves of window CTAs
+    // (4 per SM), where the flush of one half runs under the other half's partial last wave; larger crowds fill the
+    // GPU with every kernel and smaller ones must not be shortened further.
+    const int slots = 4 * c->n_sm;
+    const int want = c->n_sub ? c->n_sub : (d.W > slots && d.W <= 4 * slots ? 2 : 1);
+    const int nsub = (want > 1 && !c->profile && d.W >= 2 * want) ? want : 1;
     cudaStream_t s0 = c->stream;
     if (nsub > 1) {
       CUDA_TRY(cudaEventRecord(c->ev_fork, s0));
@@ -540,7 +546,12 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   c->proposed = c->flushes = c->launches = 0;
   c->sweep_host = 0;
   c->use_graph = 1;
-  c->n_sub = 1;
+  c->n_sub = 0;
+  {
+    int devid = 0;
+    c->n_sm = 148;
+    if (cudaGetDevice(&devid) == cudaSuccess) cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, devid);
+  }
   for (int i = 0; i < 4; ++i) { c->sub_stream[i] = nullptr; c->ev_join[i] = nullptr; }
   c->ev_fork = nullptr;
   c->graph_launches = c->graph_flushes = 0;
@@ -931,7 +942,7 @@ int qmc_crowd_set_option(qmc_crowd_t* c, int option, int value)
   if (option == QMC_OPT_GRAPH) { c->use_graph = value ? 1 : 0; return QMC_OK; }
   if (option == QMC_OPT_PROFILE) { c->profile = value ? 1 : 0; return QMC_OK; }
   if (option == QMC_OPT_SUBCROWDS) {
-    if (value < 1 || value > 4) return fail(QMC_ERR_INVALID_ARG, "sub-crowds must be in [1,4]");
+    if (value < 0 || value > 4) return fail(QMC_ERR_INVALID_ARG, "sub-crowds must be in [0,4] (0 = automatic)");
     c->n_sub = value;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     return QMC_OK;
