@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--sub-crowds", type=int, default=None, help="sub-crowds qmc_sweep runs on separate streams (1..4)")
     ap.add_argument("--multi-crowd", action="store_true",
                     help="also time C crowds of W/C walkers, one stream and one host thread each (PAPER.md Alg. 4)")
+    ap.add_argument("--drift", action="store_true",
+                    help="also print the drift of the carried inverses against a recompute after 1..100 sweeps")
     ap.add_argument("--no-probes", action="store_true", help="skip the step-call / rank-1 kernel probes")
     ap.add_argument("--ref-walkers", type=int, default=None, help="walkers of the oracle sample (default = cores)")
     return ap.parse_args()
@@ -284,6 +286,31 @@ def time_multi_crowd(wl, W, C, kd, coefs_dev, dev, steps=2, warmup=1):
     return e0.elapsed_time(e1), prop, acc
 
 
+def drift_study(wl, coefs_dev, dev, W=128, ranks=(1, 32, 64), marks=(1, 5, 10, 20, 50, 100)):
+    """Round-off drift of the carried inverses: after S free-running sweeps, the largest and
+    median norm-wise difference between a walker's carried inverse and the one recomputed at the same positions."""
+    import torch
+    import paper_2209_14487_b200 as q
+    pos = torch.from_numpy(np.ascontiguousarray(qi.make_positions(wl, W))).to(dev)
+    for kd in ranks:
+        mk = lambda: q.Crowd(coefs_dev, wl.box, pos, tau=wl.tau, delay_rank=kd, j2_a=wl.j2_a, j2_b=wl.j2_b, seed=wl.seed)
+        c, f = mk(), mk()
+        done = 0
+        for S in marks:
+            c.qmc_sweep(S - done)
+            done = S
+            f.set_positions(c.positions())
+            worst, med = 0.0, 0.0
+            for spin in (0, 1):
+                B, F = c.inverse(spin), f.inverse(spin)
+                rel = (B - F).abs().amax(dim=(1, 2)) / F.abs().amax(dim=(1, 2))
+                worst, med = max(worst, float(rel.max())), max(med, float(rel.median()))
+            print(json.dumps({"drift": True, "walkers": W, "delay_rank": kd, "sweeps": S, "rel_diff_max": worst,
+                              "rel_diff_median": med}), flush=True)
+        c.close()
+        f.close()
+
+
 def ncu_traffic(cfg, W, kd):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu captures
     (profiles/r1_dram_traffic.csv: cfg,walkers,delay_rank,kernel,bytes), for the configuration timed here."""
@@ -506,6 +533,8 @@ def run_cuda(args):
                 c2.close()
                 del c2
                 torch.cuda.empty_cache()
+    if args.drift and world == 1:
+        drift_study(wl, coefs_dev, dev)
     if args.multi_crowd and world == 1:
         # S:8(f) item 1: does splitting a crowd of W into C crowds on C streams / host threads pay at small W?
         for W2 in (256, 512, 1024, 4096):

@@ -143,6 +143,16 @@ int qmc_sweep_host(qmc_crowd_t* crowd, double* pos_host, int n_sweeps, uint64_t*
  * (call qmc_flush_delayed first; qmc_sweep always returns flushed).                                              */
 int qmc_kinetic_energy(qmc_crowd_t* crowd, double* ekin_dev, double* e_elec_dev);
 
+/* Periodic recompute of the inverses (first half; the usual answer to the round-off drift of
+ * repeated Sherman-Morrison / delayed updates; "update the internal data of a walker" names
+ * the carried data this replaces): rebuilds both Slater matrices of every walker from the crowd's CURRENT positions
+ * (B-spline values and the gradient / Laplacian caches of every electron), inverts them with partial pivoting in fp64
+ * and drops any open delayed window -- the same code path as qmc_crowd_create / qmc_crowd_set_positions, so the
+ * result is bit-identical to a crowd created at those positions.  Counters and the sweep index are kept.
+ * Synchronises desc.stream.  QMC_ERR_STATE in the middle of a move; QMC_ERR_SINGULAR as for qmc_crowd_create (the
+ * crowd is then unusable until qmc_crowd_set_positions succeeds).                                             */
+int qmc_recompute_inverse(qmc_crowd_t* crowd);
+
 /* ---- state access for tests: synchronous copies on desc.stream -------------------------- */
 int qmc_crowd_get_positions(qmc_crowd_t* crowd, double* pos_dev /* DEVICE [W][N][3] */);
 int qmc_crowd_set_positions(qmc_crowd_t* crowd, const double* pos_dev); /* rebuilds, may be SINGULAR */
@@ -178,6 +188,10 @@ int qmc_crowd_set_option(qmc_crowd_t* crowd, int option, int value);
  * streams when delay_rank > 1 (crowds on independent streams overlap); walkers are independent, so
  * results do not depend on it.  The sub-crowds are forked from and joined back into desc.stream every sweep.    */
 #define QMC_OPT_SUBCROWDS 2
+/* option 3 (QMC_OPT_RECOMPUTE_EVERY): qmc_sweep / qmc_sweep_host call qmc_recompute_inverse after every `value`-th
+ * sweep (counted on the crowd's sweep index, so the schedule does not depend on how sweeps are batched into calls);
+ * 0 = never (default).                                                                                          */
+#define QMC_OPT_RECOMPUTE_EVERY 3
 
 /* kernel classes of the hot path, index into qmc_crowd_get_profile's arrays */
 enum {

@@ -17,12 +17,13 @@ QMC_OK, QMC_ERR_INVALID_ARG, QMC_ERR_CUDA, QMC_ERR_WORKSPACE, QMC_ERR_SINGULAR, 
 QMC_OPT_GRAPH = 0
 QMC_OPT_PROFILE = 1
 QMC_OPT_SUBCROWDS = 2
+QMC_OPT_RECOMPUTE_EVERY = 3
 KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush", "ratio_accept",
                   "fused_move", "window", "kinetic")
 
 EXPORTS = [
     "qmc_crowd_workspace_bytes", "qmc_crowd_create", "qmc_crowd_destroy", "qmc_spo_vgl", "qmc_ratio_grad",
-    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_kinetic_energy", "qmc_crowd_get_positions",
+    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_kinetic_energy", "qmc_recompute_inverse", "qmc_crowd_get_positions",
     "qmc_crowd_set_positions", "qmc_crowd_get_inverse", "qmc_crowd_set_inverse", "qmc_crowd_get_caches",
     "qmc_crowd_get_window", "qmc_crowd_get_move", "qmc_crowd_set_sweep_index", "qmc_crowd_stats",
     "qmc_crowd_launch_count", "qmc_crowd_set_option", "qmc_crowd_get_profile", "qmc_last_error", "qmc_version",
@@ -71,6 +72,7 @@ def load():
     L.qmc_ratio_grad.argtypes = [vp, ip, dp, dp]
     L.qmc_accept_reject.argtypes = [vp, ip, vp]
     L.qmc_flush_delayed.argtypes = [vp]
+    L.qmc_recompute_inverse.argtypes = [vp]
     L.qmc_sweep.argtypes = [vp, ip]
     L.qmc_sweep_host.argtypes = [vp, vp, ip, vp]
     L.qmc_kinetic_energy.argtypes = [vp, dp, dp]
@@ -178,6 +180,9 @@ class Crowd:
 
     def qmc_flush_delayed(self):
         _check(load().qmc_flush_delayed(self._h))
+
+    def qmc_recompute_inverse(self):
+        _check(load().qmc_recompute_inverse(self._h))
 
     def qmc_sweep(self, n_sweeps=1):
         _check(load().qmc_sweep(self._h, n_sweeps))

@@ -68,6 +68,7 @@ struct qmc_crowd {
   uint32_t sweep_host;
   int use_graph;
   int n_sub;                        // sub-crowds of qmc_sweep (delay_rank > 1), each on its own stream; 0 = automatic
+  int recompute_every;              // qmc_sweep recomputes the inverses every this many sweeps (0 = never)
   int n_sm;                         // SMs of the device (sizes the automatic sub-crowd choice)
   cudaStream_t sub_stream[4];
   cudaEvent_t ev_fork, ev_join[4];
@@ -547,6 +548,7 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   c->sweep_host = 0;
   c->use_graph = 1;
   c->n_sub = 0;
+  c->recompute_every = 0;
   {
     int devid = 0;
     c->n_sm = 148;
@@ -742,8 +744,19 @@ int qmc_sweep(qmc_crowd_t* c, int n_sweeps)
     }
     c->proposed += (uint64_t)d.W * d.N;
     ++c->sweep_host;
+    if (c->recompute_every > 0 && c->sweep_host % (uint32_t)c->recompute_every == 0) {
+      st = rebuild(c);
+      if (st) return st;
+    }
   }
   return QMC_OK;
+}
+
+int qmc_recompute_inverse(qmc_crowd_t* c)
+{
+  if (!c) return fail(QMC_ERR_INVALID_ARG, "crowd is NULL");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_recompute_inverse in the middle of a move");
+  return rebuild(c);
 }
 
 int qmc_sweep_host(qmc_crowd_t* c, double* pos_host, int n_sweeps, uint64_t* stats_host)
@@ -945,6 +958,11 @@ int qmc_crowd_set_option(qmc_crowd_t* c, int option, int value)
     if (value < 0 || value > 4) return fail(QMC_ERR_INVALID_ARG, "sub-crowds must be in [0,4] (0 = automatic)");
     c->n_sub = value;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    return QMC_OK;
+  }
+  if (option == QMC_OPT_RECOMPUTE_EVERY) {
+    if (value < 0) return fail(QMC_ERR_INVALID_ARG, "recompute period must be >= 0");
+    c->recompute_every = value;
     return QMC_OK;
   }
   return fail(QMC_ERR_INVALID_ARG, "unknown option %d", option);
