@@ -201,6 +201,8 @@ def algorithmic(wl, W, kd, alpha, el, m_move=None):
         # kinetic energy: both inverses, the four cache rows of every electron, positions; ~30 fp64 flop per pair term
         # (min image, rsqrt, reciprocal, u', u'') and 8 per (electron, orbital) of the four dots
         "kinetic": {"bytes": W * (16 * n * n + 4 * N * M * el + 24 * N), "flops": W * (30.0 * N * (N - 1) + 8.0 * N * M)},
+        # branching probe: every tenth walker replaced by its neighbour; state read once and written once
+        "branch": {"bytes": 2 * (W // 10) * (16 * n * n + 4 * N * M * el + 24 * N)},
         "rank1": {"bytes": alpha * W * 16 * n * n, "flops": alpha * W * 4 * n * n},
         "flush": {"bytes": W * 16 * n * n, "flops": W * (4 * n * n * m_flush + 2 * n * m_flush ** 2)},
     }
@@ -389,6 +391,10 @@ def run_cuda(args):
         crowd.qmc_flush_delayed()
         crowd.qmc_kinetic_energy()
         crowd.qmc_kinetic_energy()
+        src = torch.arange(W, dtype=torch.int32, device=dev)
+        src[9::10] -= 1
+        crowd.qmc_crowd_branch(src)
+        crowd.qmc_crowd_branch(src)
         step_prof = {k2: v for k2, v in crowd.profile().items() if v[1] and k2 != "flush"}
     crowd.set_option(q.QMC_OPT_PROFILE, 0)
     tot_ms = sum(v[0] for v in prof.values()) or 1.0
@@ -441,7 +447,7 @@ def run_cuda(args):
         extra_rooflines["kinetic"] = {"kernel": "kinetic_kernel (qmc_kinetic_energy)", "bound": "alu", "achieved": tf,
                                       "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak, "traffic": None,
                                       "avg_us": k_["avg_us"], "hbm_frac": k_["hbm_frac"]}
-    for name in ("spline_vgl", "rank1"):
+    for name in ("spline_vgl", "rank1", "branch"):
         if name in kernels:
             extra_rooflines[name] = {"kernel": name, "bound": "hbm", "achieved": kernels[name]["gbs"],
                                      "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": kernels[name]["hbm_frac"],

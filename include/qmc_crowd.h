@@ -153,6 +153,16 @@ int qmc_kinetic_energy(qmc_crowd_t* crowd, double* ekin_dev, double* e_elec_dev)
  * crowd is then unusable until qmc_crowd_set_positions succeeds).                                             */
 int qmc_recompute_inverse(qmc_crowd_t* crowd);
 
+/* DMC branching, data movement only (Alg. 1 L13 "branch"; P:66 for the walker
+ * states it moves): walker slot w takes over the whole carried state of slot src[w] -- positions, both inverses,
+ * gradient / Laplacian caches.  src is a DEVICE int32 array of W entries, BORROWED; every source must keep its own
+ * state (src[src[w]] == src[w], which includes src[w] == w for walkers that are not replaced); an invalid map returns
+ * QMC_ERR_INVALID_ARG and changes nothing.  Random-number streams stay with the slot (PAPER.md gives no rule; D:A3
+ * keys Philox on the global walker id), so a copy diverges from its source at the next move.  Counters and the sweep
+ * index are kept; an open delayed window is flushed first.  Synchronises desc.stream (the map is validated on the
+ * device before the copy).  n_copied (HOST, may be NULL) receives the number of slots that were overwritten.    */
+int qmc_crowd_branch(qmc_crowd_t* crowd, const int32_t* src_dev, int* n_copied);
+
 /* ---- state access for tests: synchronous copies on desc.stream -------------------------- */
 int qmc_crowd_get_positions(qmc_crowd_t* crowd, double* pos_dev /* DEVICE [W][N][3] */);
 int qmc_crowd_set_positions(qmc_crowd_t* crowd, const double* pos_dev); /* rebuilds, may be SINGULAR */
@@ -205,7 +215,8 @@ enum {
   QMC_K_FUSED_MOVE = 7,  /* (no longer launched; kept so that class numbers stay stable)         */
   QMC_K_WINDOW = 8,      /* qmc_sweep: all moves of one delay window (or, delay_rank 1 and small n, of a sweep), CTA per walker */
   QMC_K_KINETIC = 9,     /* qmc_kinetic_energy                                                   */
-  QMC_N_KERNEL_CLASSES = 10
+  QMC_K_BRANCH = 10,     /* qmc_crowd_branch (state copy)                                        */
+  QMC_N_KERNEL_CLASSES = 11
 };
 /* Device time (ms, CUDA events on desc.stream) and launch count per kernel class accumulated in
  * profile mode since the previous call; resets the accumulators.  Synchronous.  ms and count

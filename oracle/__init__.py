@@ -80,6 +80,8 @@ def lib():
     L.oracle_crowd_sweep.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
     L.oracle_crowd_sweep.restype = C.c_int64
     L.oracle_crowd_set_sweep_index.argtypes = [C.c_void_p, C.c_uint32]
+    L.oracle_crowd_branch.argtypes = [C.c_void_p, C.c_void_p]
+    L.oracle_crowd_branch.restype = C.c_int
     L.oracle_crowd_get_positions.argtypes = [C.c_void_p, dp]
     L.oracle_crowd_get_inverse.argtypes = [C.c_void_p, C.c_int, dp]
     L.oracle_num_threads.restype = C.c_int
@@ -252,6 +254,13 @@ class OracleCrowd:
 
     def set_sweep_index(self, s: int):
         lib().oracle_crowd_set_sweep_index(self._h, s)
+
+    def branch(self, src):
+        src = np.ascontiguousarray(src, dtype=np.int32)
+        assert src.shape == (self.W,)
+        st = lib().oracle_crowd_branch(self._h, src.ctypes.data)
+        if st != 0:
+            raise ValueError(f"oracle_crowd_branch: status {st}")
 
     def positions(self) -> np.ndarray:
         out = np.zeros((self.W, self.sys.n_elec, 3))

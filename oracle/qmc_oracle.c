@@ -618,6 +618,35 @@ int64_t oracle_crowd_sweep(oracle_crowd* c, int n_sweeps, oracle_move_log* log)
 
 void oracle_crowd_set_sweep_index(oracle_crowd* c, uint32_t s) { c->sweep = s; }
 
+/* DMC branching, data movement only (Alg. 1 L13): walker slot w takes over every carried
+ * quantity of slot src[w].  Written as the definition: a full copy of the old state, then a gather -- no
+ * condition on src beyond its range.  Returns -1 for an entry outside [0, W) or an open delayed window. */
+int oracle_crowd_branch(oracle_crowd* c, const int32_t* src)
+{
+  const size_t W = (size_t)c->W, N = (size_t)c->N, n = (size_t)c->n, M = (size_t)c->M;
+  for (size_t w = 0; w < W; ++w)
+    if (src[w] < 0 || src[w] >= c->W || c->m[w] != 0) return -1;
+  const size_t sR = N * 3, sB = 2 * n * n, sD = N * 3 * M, sL = N * M;
+  double* R0 = (double*)malloc(sizeof(double) * W * sR);
+  double* B0 = (double*)malloc(sizeof(double) * W * sB);
+  double* D0 = (double*)malloc(sizeof(double) * W * sD);
+  double* L0 = (double*)malloc(sizeof(double) * W * sL);
+  if (!R0 || !B0 || !D0 || !L0) { free(R0); free(B0); free(D0); free(L0); return -2; }
+  memcpy(R0, c->R, sizeof(double) * W * sR);
+  memcpy(B0, c->B, sizeof(double) * W * sB);
+  memcpy(D0, c->dphi, sizeof(double) * W * sD);
+  memcpy(L0, c->d2phi, sizeof(double) * W * sL);
+  for (size_t w = 0; w < W; ++w) {
+    const size_t s = (size_t)src[w];
+    memcpy(c->R + w * sR, R0 + s * sR, sizeof(double) * sR);
+    memcpy(c->B + w * sB, B0 + s * sB, sizeof(double) * sB);
+    memcpy(c->dphi + w * sD, D0 + s * sD, sizeof(double) * sD);
+    memcpy(c->d2phi + w * sL, L0 + s * sL, sizeof(double) * sL);
+  }
+  free(R0); free(B0); free(D0); free(L0);
+  return 0;
+}
+
 void oracle_crowd_get_positions(const oracle_crowd* c, double* pos)
 {
   memcpy(pos, c->R, sizeof(double) * (size_t)c->W * c->N * 3);

@@ -116,6 +116,8 @@ void oracle_crowd_destroy(oracle_crowd* c);
  * [n_sweeps][W][N] records. Returns number of accepted moves. Threads over walkers. */
 int64_t oracle_crowd_sweep(oracle_crowd* c, int n_sweeps, oracle_move_log* log);
 void oracle_crowd_set_sweep_index(oracle_crowd* c, uint32_t s);
+/* branching data movement: slot w <- state of slot src[w]; -1 on a bad entry / open window */
+int  oracle_crowd_branch(oracle_crowd* c, const int32_t* src /*[W]*/);
 void oracle_crowd_get_positions(const oracle_crowd* c, double* pos /*[W][N][3]*/);
 void oracle_crowd_get_inverse(const oracle_crowd* c, int spin, double* B /*[W][n][n]*/);
 int  oracle_num_threads(void);

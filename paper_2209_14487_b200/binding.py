@@ -19,11 +19,11 @@ QMC_OPT_PROFILE = 1
 QMC_OPT_SUBCROWDS = 2
 QMC_OPT_RECOMPUTE_EVERY = 3
 KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush", "ratio_accept",
-                  "fused_move", "window", "kinetic")
+                  "fused_move", "window", "kinetic", "branch")
 
 EXPORTS = [
     "qmc_crowd_workspace_bytes", "qmc_crowd_create", "qmc_crowd_destroy", "qmc_spo_vgl", "qmc_ratio_grad",
-    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_kinetic_energy", "qmc_recompute_inverse", "qmc_crowd_get_positions",
+    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_kinetic_energy", "qmc_recompute_inverse", "qmc_crowd_branch", "qmc_crowd_get_positions",
     "qmc_crowd_set_positions", "qmc_crowd_get_inverse", "qmc_crowd_set_inverse", "qmc_crowd_get_caches",
     "qmc_crowd_get_window", "qmc_crowd_get_move", "qmc_crowd_set_sweep_index", "qmc_crowd_stats",
     "qmc_crowd_launch_count", "qmc_crowd_set_option", "qmc_crowd_get_profile", "qmc_last_error", "qmc_version",
@@ -73,6 +73,7 @@ def load():
     L.qmc_accept_reject.argtypes = [vp, ip, vp]
     L.qmc_flush_delayed.argtypes = [vp]
     L.qmc_recompute_inverse.argtypes = [vp]
+    L.qmc_crowd_branch.argtypes = [vp, vp, C.POINTER(C.c_int)]
     L.qmc_sweep.argtypes = [vp, ip]
     L.qmc_sweep_host.argtypes = [vp, vp, ip, vp]
     L.qmc_kinetic_energy.argtypes = [vp, dp, dp]
@@ -183,6 +184,15 @@ class Crowd:
 
     def qmc_recompute_inverse(self):
         _check(load().qmc_recompute_inverse(self._h))
+
+    def qmc_crowd_branch(self, src):
+        """src: int32 CUDA tensor [W]; slot w takes over the state of slot src[w]. Returns the number of copied slots."""
+        import torch
+        assert src.dtype == torch.int32 and src.is_cuda and src.is_contiguous() and src.numel() == self.W
+        n = C.c_int(0)
+        with torch.cuda.stream(self.stream):
+            _check(load().qmc_crowd_branch(self._h, src.data_ptr(), C.byref(n)))
+        return n.value
 
     def qmc_sweep(self, n_sweeps=1):
         _check(load().qmc_sweep(self._h, n_sweeps))

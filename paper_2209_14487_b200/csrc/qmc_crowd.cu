@@ -18,6 +18,7 @@
 #include "energy.cuh"
 #include "update.cuh"
 #include "window.cuh"
+#include "branch.cuh"
 
 using namespace qmc;
 
@@ -903,6 +904,48 @@ int qmc_kinetic_energy(qmc_crowd_t* c, double* ekin_dev, double* e_elec_dev)
     LAUNCH_CHECK(c);
   }
   if (e_elec_dev) CUDA_TRY(cudaMemcpyAsync(e_elec_dev, d.e_elec, (size_t)d.W * d.N * 8, cudaMemcpyDeviceToDevice, c->stream));
+  return QMC_OK;
+}
+
+__global__ void branch_count_kernel(int W, const int* __restrict__ src, int* out)
+{
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned b = __ballot_sync(0xffffffffu, w < W && src[w] != w);
+  if ((threadIdx.x & 31) == 0 && b) atomicAdd(out, __popc(b));
+}
+
+int qmc_crowd_branch(qmc_crowd_t* c, const int32_t* src_dev, int* n_copied)
+{
+  if (!c || !src_dev) return fail(QMC_ERR_INVALID_ARG, "NULL argument");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_crowd_branch in the middle of a move");
+  int st = qmc_flush_delayed(c);
+  if (st) return st;
+  const CrowdDev& d = c->dev;
+  // validate the map on the device; d.status doubles as the flag, d.mwin[0] (zero: the window is empty) as the counter
+  CUDA_TRY(cudaMemsetAsync(d.status, 0, 4, c->stream));
+  branch_check_kernel<<<(d.W + 255) / 256, 256, 0, c->stream>>>(d, src_dev);
+  LAUNCH_CHECK(c);
+  branch_count_kernel<<<(d.W + 255) / 256, 256, 0, c->stream>>>(d.W, src_dev, d.mwin);
+  LAUNCH_CHECK(c);
+  int flag = 0, cnt = 0;
+  CUDA_TRY(cudaMemcpyAsync(&flag, d.status, 4, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(cudaMemcpyAsync(&cnt, d.mwin, 4, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(cudaMemsetAsync(d.status, 0, 4, c->stream));
+  CUDA_TRY(cudaMemsetAsync(d.mwin, 0, 4, c->stream));
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  if (flag) return fail(QMC_ERR_INVALID_ARG, "src is not a branching map: entries must lie in [0, W) and sources must keep their own state");
+  if (n_copied) *n_copied = cnt;
+  if (cnt == 0) return QMC_OK;
+  {
+    ProfScope ps(c, QMC_K_BRANCH);
+    const size_t cache_bytes = (size_t)d.N * 4 * d.ns * c->elem;
+    const size_t vecs = ((size_t)2 * d.ns * d.ns * 8 + cache_bytes) / 16;
+    int chunks = (int)((vecs + (size_t)BRANCH_NT * 32 - 1) / ((size_t)BRANCH_NT * 32));  // ~32 vectors per thread
+    if (chunks < 1) chunks = 1;
+    if (chunks > 64) chunks = 64;
+    branch_copy_kernel<<<dim3(chunks, d.W), BRANCH_NT, 0, c->stream>>>(d, src_dev, cache_bytes);
+    LAUNCH_CHECK(c);
+  }
   return QMC_OK;
 }
 
