@@ -163,6 +163,19 @@ int qmc_recompute_inverse(qmc_crowd_t* crowd);
  * device before the copy).  n_copied (HOST, may be NULL) receives the number of slots that were overwritten.    */
 int qmc_crowd_branch(qmc_crowd_t* crowd, const int32_t* src_dev, int* n_copied);
 
+/* Walker states as messages (second half; the DMC load balance of Alg. 1 L14,
+ * PAPER.md:66, P:71 moves whole walkers between ranks).  A packed state is qmc_crowd_walker_state_bytes(crowd) bytes:
+ * [both inverses, fp64 [2][ns][ns] | gradient / Laplacian caches, table dtype [N][4][ns] | positions, fp64 [N][3]];
+ * it can be imported only into a crowd created with the same n_elec, n_orb and coefficient dtype (same byte count).
+ * export: buf[i] <- state of slot slots[i]; import: slot slots[i] <- buf[i], i < n.  slots: DEVICE int32 [n], in
+ * [0, W) and distinct (else QMC_ERR_INVALID_ARG, nothing copied); buf: DEVICE, 16-byte aligned, n packed states,
+ * BORROWED.  An open delayed window is flushed first; the validation synchronises desc.stream, the copy itself is
+ * asynchronous on it.  The transport between ranks is the caller's (paper_2209_14487_b200/dist.py sends the packed
+ * buffers point-to-point on the NCCL backend).                                                                 */
+size_t qmc_crowd_walker_state_bytes(const qmc_crowd_t* crowd);
+int qmc_crowd_export_walkers(qmc_crowd_t* crowd, int n, const int32_t* slots_dev, void* buf_dev);
+int qmc_crowd_import_walkers(qmc_crowd_t* crowd, int n, const int32_t* slots_dev, const void* buf_dev);
+
 /* ---- state access for tests: synchronous copies on desc.stream -------------------------- */
 int qmc_crowd_get_positions(qmc_crowd_t* crowd, double* pos_dev /* DEVICE [W][N][3] */);
 int qmc_crowd_set_positions(qmc_crowd_t* crowd, const double* pos_dev); /* rebuilds, may be SINGULAR */
@@ -215,7 +228,7 @@ enum {
   QMC_K_FUSED_MOVE = 7,  /* (no longer launched; kept so that class numbers stay stable)         */
   QMC_K_WINDOW = 8,      /* qmc_sweep: all moves of one delay window (or, delay_rank 1 and small n, of a sweep), CTA per walker */
   QMC_K_KINETIC = 9,     /* qmc_kinetic_energy                                                   */
-  QMC_K_BRANCH = 10,     /* qmc_crowd_branch (state copy)                                        */
+  QMC_K_BRANCH = 10,     /* qmc_crowd_branch, qmc_crowd_export / import_walkers (state copies)   */
   QMC_N_KERNEL_CLASSES = 11
 };
 /* Device time (ms, CUDA events on desc.stream) and launch count per kernel class accumulated in

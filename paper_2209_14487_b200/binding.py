@@ -23,7 +23,8 @@ KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", 
 
 EXPORTS = [
     "qmc_crowd_workspace_bytes", "qmc_crowd_create", "qmc_crowd_destroy", "qmc_spo_vgl", "qmc_ratio_grad",
-    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_kinetic_energy", "qmc_recompute_inverse", "qmc_crowd_branch", "qmc_crowd_get_positions",
+    "qmc_accept_reject", "qmc_flush_delayed", "qmc_sweep", "qmc_sweep_host", "qmc_kinetic_energy", "qmc_recompute_inverse", "qmc_crowd_branch", "qmc_crowd_walker_state_bytes", "qmc_crowd_export_walkers",
+    "qmc_crowd_import_walkers", "qmc_crowd_get_positions",
     "qmc_crowd_set_positions", "qmc_crowd_get_inverse", "qmc_crowd_set_inverse", "qmc_crowd_get_caches",
     "qmc_crowd_get_window", "qmc_crowd_get_move", "qmc_crowd_set_sweep_index", "qmc_crowd_stats",
     "qmc_crowd_launch_count", "qmc_crowd_set_option", "qmc_crowd_get_profile", "qmc_last_error", "qmc_version",
@@ -74,6 +75,10 @@ def load():
     L.qmc_flush_delayed.argtypes = [vp]
     L.qmc_recompute_inverse.argtypes = [vp]
     L.qmc_crowd_branch.argtypes = [vp, vp, C.POINTER(C.c_int)]
+    L.qmc_crowd_walker_state_bytes.argtypes = [vp]
+    L.qmc_crowd_walker_state_bytes.restype = C.c_size_t
+    L.qmc_crowd_export_walkers.argtypes = [vp, ip, vp, vp]
+    L.qmc_crowd_import_walkers.argtypes = [vp, ip, vp, vp]
     L.qmc_sweep.argtypes = [vp, ip]
     L.qmc_sweep_host.argtypes = [vp, vp, ip, vp]
     L.qmc_kinetic_energy.argtypes = [vp, dp, dp]
@@ -184,6 +189,28 @@ class Crowd:
 
     def qmc_recompute_inverse(self):
         _check(load().qmc_recompute_inverse(self._h))
+
+    def walker_state_bytes(self):
+        return int(load().qmc_crowd_walker_state_bytes(self._h))
+
+    def qmc_crowd_export_walkers(self, slots):
+        """slots: int32 CUDA tensor [n]. Returns a uint8 CUDA tensor [n, walker_state_bytes] of packed states."""
+        import torch
+        assert slots.dtype == torch.int32 and slots.is_cuda and slots.is_contiguous()
+        n = slots.numel()
+        buf = torch.empty((n, self.walker_state_bytes()), dtype=torch.uint8, device=self.device)
+        with torch.cuda.stream(self.stream):
+            _check(load().qmc_crowd_export_walkers(self._h, n, slots.data_ptr(), buf.data_ptr()))
+        return buf
+
+    def qmc_crowd_import_walkers(self, slots, buf):
+        import torch
+        assert slots.dtype == torch.int32 and slots.is_cuda and slots.is_contiguous()
+        n = slots.numel()
+        assert buf.dtype == torch.uint8 and buf.is_cuda and buf.is_contiguous()
+        assert buf.numel() == n * self.walker_state_bytes()
+        with torch.cuda.stream(self.stream):
+            _check(load().qmc_crowd_import_walkers(self._h, n, slots.data_ptr(), buf.data_ptr()))
 
     def qmc_crowd_branch(self, src):
         """src: int32 CUDA tensor [W]; slot w takes over the state of slot src[w]. Returns the number of copied slots."""

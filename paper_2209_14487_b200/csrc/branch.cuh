@@ -23,68 +23,85 @@ __global__ void branch_check_kernel(CrowdDev d, const int* __restrict__ src)
   if (s < 0 || s >= d.W || src[s] != s) atomicOr(d.status, 8);
 }
 
+// 16-byte streaming copy of nvec vectors, strided over the grid's x dimension, four loads in flight per thread
+__device__ __forceinline__ void stream_copy16(double* dp, const double* sp, size_t nvec, unsigned long long pol)
+{
+  const size_t stride = (size_t)gridDim.x * BRANCH_NT;
+  size_t i = (size_t)blockIdx.x * BRANCH_NT + threadIdx.x;
+  for (; i + 3 * stride < nvec; i += 4 * stride) {
+    double v0[2], v1[2], v2[2], v3[2];
+    ld16_stream(sp + 2 * i, v0, pol);
+    ld16_stream(sp + 2 * (i + stride), v1, pol);
+    ld16_stream(sp + 2 * (i + 2 * stride), v2, pol);
+    ld16_stream(sp + 2 * (i + 3 * stride), v3, pol);
+    st16(dp + 2 * i, v0);
+    st16(dp + 2 * (i + stride), v1);
+    st16(dp + 2 * (i + 2 * stride), v2);
+    st16(dp + 2 * (i + 3 * stride), v3);
+  }
+  for (; i < nvec; i += stride) {
+    double v[2];
+    ld16_stream(sp + 2 * i, v, pol);
+    st16(dp + 2 * i, v);
+  }
+}
+
+// The carried state of one walker as three byte ranges (all multiples of 16 bytes: ns, N are even).
+struct WalkerState {
+  size_t inv_bytes, cache_bytes, pos_bytes;
+  __host__ __device__ size_t total() const { return inv_bytes + cache_bytes + pos_bytes; }
+};
+__host__ __device__ inline WalkerState walker_state(const CrowdDev& d, size_t elem)
+{
+  return WalkerState{(size_t)2 * d.ns * d.ns * 8, (size_t)d.N * 4 * d.ns * elem, (size_t)d.N * 3 * 8};
+}
+
 // grid = (chunks, W): CTA (c, w) copies its share of the three state arrays of walker src[w] into walker w
-__global__ void __launch_bounds__(BRANCH_NT) branch_copy_kernel(CrowdDev d, const int* __restrict__ src,
-                                                                size_t cache_bytes_per_walker)
+__global__ void __launch_bounds__(BRANCH_NT) branch_copy_kernel(CrowdDev d, const int* __restrict__ src, WalkerState ws)
 {
   const int w = blockIdx.y, s = src[w];
   if (s == w) return;
   const unsigned long long pol = l2_evict_first_policy();
-  const size_t n_inv = (size_t)2 * d.ns * d.ns / 2;          // 16-byte vectors of the two inverses
-  const size_t n_cache = cache_bytes_per_walker / 16;
-  const size_t n_pos = ((size_t)d.N * 3) / 2;                // N is even: 3 N doubles = 3 N / 2 vectors
-  const size_t tid = (size_t)blockIdx.x * BRANCH_NT + threadIdx.x, stride = (size_t)gridDim.x * BRANCH_NT;
-  {
-    const double* sp = d.Binv + (size_t)s * n_inv * 2;
-    double* dp = d.Binv + (size_t)w * n_inv * 2;
-    size_t i = tid;
-    for (; i + 3 * stride < n_inv; i += 4 * stride) {  // four independent 16-byte loads in flight per thread
-      double v0[2], v1[2], v2[2], v3[2];
-      ld16_stream(sp + 2 * i, v0, pol);
-      ld16_stream(sp + 2 * (i + stride), v1, pol);
-      ld16_stream(sp + 2 * (i + 2 * stride), v2, pol);
-      ld16_stream(sp + 2 * (i + 3 * stride), v3, pol);
-      st16(dp + 2 * i, v0);
-      st16(dp + 2 * (i + stride), v1);
-      st16(dp + 2 * (i + 2 * stride), v2);
-      st16(dp + 2 * (i + 3 * stride), v3);
-    }
-    for (; i < n_inv; i += stride) {
-      double v[2];
-      ld16_stream(sp + 2 * i, v, pol);
-      st16(dp + 2 * i, v);
-    }
+  stream_copy16(d.Binv + (size_t)w * (ws.inv_bytes / 8), d.Binv + (size_t)s * (ws.inv_bytes / 8), ws.inv_bytes / 16, pol);
+  stream_copy16(reinterpret_cast<double*>(static_cast<char*>(d.cache) + (size_t)w * ws.cache_bytes),
+                reinterpret_cast<const double*>(static_cast<const char*>(d.cache) + (size_t)s * ws.cache_bytes),
+                ws.cache_bytes / 16, pol);
+  stream_copy16(d.R + (size_t)w * (ws.pos_bytes / 8), d.R + (size_t)s * (ws.pos_bytes / 8), ws.pos_bytes / 16, pol);
+}
+
+// Walker states to / from a packed buffer (the message of the DMC load balance, Alg. 1 L14):
+// buf[i] = [inverses | caches | positions] of walker slots[i] (EXPORT) or the reverse (IMPORT).  grid = (chunks, n).
+template <bool EXPORT>
+__global__ void __launch_bounds__(BRANCH_NT) walker_pack_kernel(CrowdDev d, const int* __restrict__ slots, char* buf,
+                                                                WalkerState ws)
+{
+  const int i = blockIdx.y, w = slots[i];
+  const unsigned long long pol = l2_evict_first_policy();
+  double* b_inv = reinterpret_cast<double*>(buf + (size_t)i * ws.total());
+  double* b_cache = reinterpret_cast<double*>(buf + (size_t)i * ws.total() + ws.inv_bytes);
+  double* b_pos = reinterpret_cast<double*>(buf + (size_t)i * ws.total() + ws.inv_bytes + ws.cache_bytes);
+  double* w_inv = d.Binv + (size_t)w * (ws.inv_bytes / 8);
+  double* w_cache = reinterpret_cast<double*>(static_cast<char*>(d.cache) + (size_t)w * ws.cache_bytes);
+  double* w_pos = d.R + (size_t)w * (ws.pos_bytes / 8);
+  if (EXPORT) {
+    stream_copy16(b_inv, w_inv, ws.inv_bytes / 16, pol);
+    stream_copy16(b_cache, w_cache, ws.cache_bytes / 16, pol);
+    stream_copy16(b_pos, w_pos, ws.pos_bytes / 16, pol);
+  } else {
+    stream_copy16(w_inv, b_inv, ws.inv_bytes / 16, pol);
+    stream_copy16(w_cache, b_cache, ws.cache_bytes / 16, pol);
+    stream_copy16(w_pos, b_pos, ws.pos_bytes / 16, pol);
   }
-  {
-    const double* sp = reinterpret_cast<const double*>(static_cast<const char*>(d.cache) + (size_t)s * cache_bytes_per_walker);
-    double* dp = reinterpret_cast<double*>(static_cast<char*>(d.cache) + (size_t)w * cache_bytes_per_walker);
-    size_t i = tid;
-    for (; i + 3 * stride < n_cache; i += 4 * stride) {
-      double v0[2], v1[2], v2[2], v3[2];
-      ld16_stream(sp + 2 * i, v0, pol);
-      ld16_stream(sp + 2 * (i + stride), v1, pol);
-      ld16_stream(sp + 2 * (i + 2 * stride), v2, pol);
-      ld16_stream(sp + 2 * (i + 3 * stride), v3, pol);
-      st16(dp + 2 * i, v0);
-      st16(dp + 2 * (i + stride), v1);
-      st16(dp + 2 * (i + 2 * stride), v2);
-      st16(dp + 2 * (i + 3 * stride), v3);
-    }
-    for (; i < n_cache; i += stride) {
-      double v[2];
-      ld16_stream(sp + 2 * i, v, pol);
-      st16(dp + 2 * i, v);
-    }
-  }
-  {
-    const double* sp = d.R + (size_t)s * d.N * 3;
-    double* dp = d.R + (size_t)w * d.N * 3;
-    for (size_t i = tid; i < n_pos; i += stride) {
-      double v[2];
-      ld16_stream(sp + 2 * i, v, pol);
-      st16(dp + 2 * i, v);
-    }
-  }
+}
+
+// status |= 8 for a slot outside [0, W) or listed twice (marks: W zeroed ints, left dirty -- the caller clears them)
+__global__ void slots_check_kernel(CrowdDev d, int n, const int* __restrict__ slots, int* marks)
+{
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int w = slots[i];
+  if (w < 0 || w >= d.W) { atomicOr(d.status, 8); return; }
+  if (atomicAdd(marks + w, 1) != 0) atomicOr(d.status, 8);
 }
 
 }  // namespace qmc

@@ -907,6 +907,14 @@ int qmc_kinetic_energy(qmc_crowd_t* c, double* ekin_dev, double* e_elec_dev)
   return QMC_OK;
 }
 
+// CTAs per walker of the state copies: about 32 16-byte vectors per thread
+int state_chunks(const WalkerState& ws)
+{
+  const size_t vecs = ws.total() / 16;
+  int chunks = (int)((vecs + (size_t)BRANCH_NT * 32 - 1) / ((size_t)BRANCH_NT * 32));
+  return chunks < 1 ? 1 : (chunks > 64 ? 64 : chunks);
+}
+
 __global__ void branch_count_kernel(int W, const int* __restrict__ src, int* out)
 {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
@@ -938,15 +946,57 @@ int qmc_crowd_branch(qmc_crowd_t* c, const int32_t* src_dev, int* n_copied)
   if (cnt == 0) return QMC_OK;
   {
     ProfScope ps(c, QMC_K_BRANCH);
-    const size_t cache_bytes = (size_t)d.N * 4 * d.ns * c->elem;
-    const size_t vecs = ((size_t)2 * d.ns * d.ns * 8 + cache_bytes) / 16;
-    int chunks = (int)((vecs + (size_t)BRANCH_NT * 32 - 1) / ((size_t)BRANCH_NT * 32));  // ~32 vectors per thread
-    if (chunks < 1) chunks = 1;
-    if (chunks > 64) chunks = 64;
-    branch_copy_kernel<<<dim3(chunks, d.W), BRANCH_NT, 0, c->stream>>>(d, src_dev, cache_bytes);
+    const WalkerState ws = walker_state(d, c->elem);
+    branch_copy_kernel<<<dim3(state_chunks(ws), d.W), BRANCH_NT, 0, c->stream>>>(d, src_dev, ws);
     LAUNCH_CHECK(c);
   }
   return QMC_OK;
+}
+
+size_t qmc_crowd_walker_state_bytes(const qmc_crowd_t* c)
+{
+  if (!c) return 0;
+  return walker_state(c->dev, c->elem).total();
+}
+
+namespace {
+int walker_pack(qmc_crowd_t* c, int n, const int32_t* slots_dev, void* buf_dev, bool do_export)
+{
+  if (!c || n < 0 || (n > 0 && (!slots_dev || !buf_dev))) return fail(QMC_ERR_INVALID_ARG, "bad argument");
+  if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "walker export / import in the middle of a move");
+  if (((uintptr_t)buf_dev & 15) != 0) return fail(QMC_ERR_INVALID_ARG, "buffer must be 16-byte aligned");
+  int st = qmc_flush_delayed(c);
+  if (st) return st;
+  const CrowdDev& d = c->dev;
+  if (n == 0) return QMC_OK;
+  if (n > d.W) return fail(QMC_ERR_INVALID_ARG, "more slots than walkers");
+  // slots must be in range and distinct; d.mwin (all zero: the window is empty) holds the marks
+  CUDA_TRY(cudaMemsetAsync(d.status, 0, 4, c->stream));
+  slots_check_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(d, n, slots_dev, d.mwin);
+  LAUNCH_CHECK(c);
+  int flag = 0;
+  CUDA_TRY(cudaMemcpyAsync(&flag, d.status, 4, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(cudaMemsetAsync(d.status, 0, 4, c->stream));
+  CUDA_TRY(cudaMemsetAsync(d.mwin, 0, (size_t)d.W * 4, c->stream));
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  if (flag) return fail(QMC_ERR_INVALID_ARG, "slots must lie in [0, W) and be distinct");
+  ProfScope ps(c, QMC_K_BRANCH);
+  const WalkerState ws = walker_state(d, c->elem);
+  if (do_export) walker_pack_kernel<true><<<dim3(state_chunks(ws), n), BRANCH_NT, 0, c->stream>>>(d, slots_dev, (char*)buf_dev, ws);
+  else walker_pack_kernel<false><<<dim3(state_chunks(ws), n), BRANCH_NT, 0, c->stream>>>(d, slots_dev, (char*)buf_dev, ws);
+  LAUNCH_CHECK(c);
+  return QMC_OK;
+}
+}  // namespace
+
+int qmc_crowd_export_walkers(qmc_crowd_t* c, int n, const int32_t* slots_dev, void* buf_dev)
+{
+  return walker_pack(c, n, slots_dev, buf_dev, true);
+}
+
+int qmc_crowd_import_walkers(qmc_crowd_t* c, int n, const int32_t* slots_dev, const void* buf_dev)
+{
+  return walker_pack(c, n, slots_dev, const_cast<void*>(buf_dev), false);
 }
 
 int qmc_crowd_set_sweep_index(qmc_crowd_t* c, uint32_t s)

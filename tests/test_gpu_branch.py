@@ -88,3 +88,52 @@ def test_branch_flushes_an_open_window_first():
     for s in (0, 1):
         assert np.array_equal(npy(a.inverse(s)), npy(b.inverse(s)))
     assert np.array_equal(npy(a.positions()), npy(b.positions()))
+
+
+def test_export_import_moves_walkers_between_crowds():
+    """qmc_crowd_export_walkers / import_walkers (the load-balance message): walkers exported from crowd A
+    and imported into crowd B carry their whole state; B then equals, slot by slot, the oracle crowd whose slots were
+    filled by oracle_crowd_branch from the same sources (the two crowds here are two halves of one global crowd)."""
+    import torch
+    import paper_2209_14487_b200 as q
+    wl = qi.small_workload(n_elec=32, grid=10, box=6.0, coef_dtype="f64", coef_dist="normal", n_walkers=8, tau=0.02,
+                           delay_rank=8, cfg=35)
+    full, osys, coefs, pos = make_pair(wl)                       # only for coefs / positions / oracle system
+    full.close()
+    A, _, _, _ = make_pair(wl, coefs=coefs, pos=pos[:4])                    # global walkers 0..3
+    B, _, _, _ = make_pair(wl, coefs=coefs, pos=pos[4:], walker_id0=4)      # global walkers 4..7
+    oc = oracle.OracleCrowd(osys, pos)                                      # all eight
+    A.qmc_sweep(2)
+    B.qmc_sweep(2)
+    oc.sweep(2)
+    nbytes = A.walker_state_bytes()
+    n = wl.n_elec // 2
+    assert nbytes == B.walker_state_bytes() == 2 * n * n * 8 + wl.n_elec * 4 * n * 8 + wl.n_elec * 24
+    buf = A.qmc_crowd_export_walkers(_i32([3, 1]))
+    assert tuple(buf.shape) == (2, nbytes)
+    RA = npy(A.positions())
+    # the tail of a packed state is the walker's positions, its head the spin-up inverse
+    assert np.array_equal(buf[0, -wl.n_elec * 24:].cpu().numpy().view(np.float64).reshape(-1, 3), RA[3])
+    assert np.array_equal(buf[1, :n * n * 8].cpu().numpy().view(np.float64).reshape(n, n), npy(A.inverse(0))[1])
+    B.qmc_crowd_import_walkers(_i32([0, 2]), buf)                # global slots 4 and 6 <- global walkers 3 and 1
+    oc.branch(np.array([0, 1, 2, 3, 3, 5, 1, 7], dtype=np.int32))
+    assert np.array_equal(npy(B.positions()), oc.positions()[4:])
+    for s in (0, 1):
+        Bo = oc.inverse(s)[4:]
+        assert np.abs(npy(B.inverse(s)) - Bo).max() <= 1e-10 * np.abs(Bo).max()
+    A.qmc_sweep(1)
+    B.qmc_sweep(1)
+    oc.sweep(1)
+    assert np.array_equal(npy(A.positions()), oc.positions()[:4])
+    assert np.array_equal(npy(B.positions()), oc.positions()[4:])
+    # refused: duplicate or out-of-range slots, nothing copied
+    R0 = npy(B.positions()).copy()
+    for bad in ([1, 1], [0, 4], [-1, 2]):
+        with pytest.raises(q.QmcError):
+            B.qmc_crowd_import_walkers(_i32(bad), buf)
+        with pytest.raises(q.QmcError):
+            B.qmc_crowd_export_walkers(_i32(bad))
+    assert np.array_equal(npy(B.positions()), R0)
+    B.qmc_sweep(1)   # still usable: marks and flags were cleared
+    assert B.qmc_crowd_export_walkers(_i32([])).shape[0] == 0
+    del torch
