@@ -161,6 +161,40 @@ __device__ __forceinline__ void block_sum_t0(double (&v)[NV], double* sm)
   __syncthreads();
 }
 
+// Sum eight values over a warp; every lane gets the eight totals.  Same butterfly (and the same pairwise tree per
+// value) as block_sum_t0, followed by eight broadcasts: 17 double shuffles instead of 40.
+__device__ __forceinline__ void warp_sum8(double (&v)[8])
+{
+  const int lane = threadIdx.x & 31;
+  double b[4], c[2], e;
+  {
+    const bool hi = lane & 16;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const double keep = hi ? v[i + 4] : v[i], send = hi ? v[i] : v[i + 4];
+      b[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+  }
+  {
+    const bool hi = lane & 8;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const double keep = hi ? b[i + 2] : b[i], send = hi ? b[i] : b[i + 2];
+      c[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+  }
+  {
+    const bool hi = lane & 4;
+    const double keep = hi ? c[1] : c[0], send = hi ? c[0] : c[1];
+    e = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+  }
+  e += __shfl_xor_sync(0xffffffffu, e, 2);
+  e += __shfl_xor_sync(0xffffffffu, e, 1);
+  // a lane holds quantity q = 4 [bit 4] + 2 [bit 3] + [bit 2]
+#pragma unroll
+  for (int q = 0; q < 8; ++q) v[q] = __shfl_sync(0xffffffffu, e, ((q >> 2) & 1) * 16 + ((q >> 1) & 1) * 8 + (q & 1) * 4);
+}
+
 // ---- Philox4x32-10 (Salmon et al., SC'11; D:C7). Counter (walker id, k, sweep, tag). ----
 __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0,
                                               unsigned k1, unsigned (&out)[4])

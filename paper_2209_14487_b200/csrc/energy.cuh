@@ -6,7 +6,10 @@
 //                   = b.lap phi + lap_k J + 2 (b.grad phi).(grad_k J) + |grad_k J|^2,
 //   grad_k J = sum_i u'(r) d/r,  lap_k J = sum_i [u''(r) + 2 u'(r)/r],  u = a r/(1 + b r)      (D:C3)
 // (the |b.grad phi|^2 of lap ln D cancels against the one in |grad ln Psi|^2).
-// One CTA per (walker, group of EKIN_EPB electrons): 4 dots of length M, N pair terms, one block sum.
+// One CTA per (walker, group of EKIN_EPB electrons), one warp per electron at a time: 4 dots of length M and N pair
+// terms strided over the lanes, one warp butterfly -- no block barrier after the positions are staged (the first
+// version reduced every electron over the whole CTA: six pair terms per thread between two barriers, 10.9 ms per
+// call at cfg 5, W = 4096).
 #pragma once
 #include "common.cuh"
 
@@ -15,25 +18,24 @@ namespace qmc {
 constexpr int EKIN_NT = 128;
 constexpr int EKIN_EPB = 8;
 
-// dynamic smem: (3 N + 32) doubles.  e_elec: [W][N] per-electron terms.
+// dynamic smem: 3 N doubles.  e_elec: [W][N] per-electron terms.
 template <typename T>
 __global__ void __launch_bounds__(EKIN_NT) kinetic_kernel(CrowdDev d, double* __restrict__ e_elec)
 {
   extern __shared__ double sm_e[];
   double* R_s = sm_e;
-  double* red = sm_e + 3 * d.N;
-  const int w = blockIdx.y, tid = threadIdx.x, ns = d.ns;
+  const int w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, ns = d.ns;
   const double* Rg = d.R + (size_t)w * d.N * 3;
   for (int j = tid; j < 3 * d.N; j += EKIN_NT) R_s[j] = Rg[j];
   __syncthreads();
   const int k_end = min((int)(blockIdx.x + 1) * EKIN_EPB, d.N);
-  for (int k = blockIdx.x * EKIN_EPB; k < k_end; ++k) {
+  for (int k = blockIdx.x * EKIN_EPB + warp; k < k_end; k += EKIN_NT / 32) {
     const int spin = k / d.n, kk = k - spin * d.n;
     const double* b = d.Binv + (((size_t)w * 2 + spin) * ns + kk) * ns;
     const T* cache = static_cast<const T*>(d.cache) + ((size_t)w * d.N + k) * 4 * ns;
     // v[0..2] = b.grad phi, v[3] = b.lap phi, v[4..6] = grad_k J, v[7] = lap_k J
     double v[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-    for (int j = tid; j < d.M; j += EKIN_NT) {
+    for (int j = lane; j < d.M; j += 32) {
       const double bj = b[j];
       v[0] = fma(bj, (double)cache[j], v[0]);
       v[1] = fma(bj, (double)cache[ns + j], v[1]);
@@ -41,7 +43,7 @@ __global__ void __launch_bounds__(EKIN_NT) kinetic_kernel(CrowdDev d, double* __
       v[3] = fma(bj, (double)cache[3 * ns + j], v[3]);
     }
     const double rk[3] = {R_s[3 * k], R_s[3 * k + 1], R_s[3 * k + 2]};
-    for (int i = tid; i < d.N; i += EKIN_NT) {
+    for (int i = lane; i < d.N; i += 32) {
       if (i == k) continue;
       double dd[3], r2 = 0.0;
 #pragma unroll
@@ -62,8 +64,8 @@ __global__ void __launch_bounds__(EKIN_NT) kinetic_kernel(CrowdDev d, double* __
         v[7] += fma(-2.0 * d.j2_b * du, inv_den, 2.0 * f);
       }
     }
-    block_sum_t0<8, EKIN_NT>(v, red);
-    if (tid == 0) {
+    warp_sum8(v);
+    if (lane == 0) {
       const double cross = v[0] * v[4] + v[1] * v[5] + v[2] * v[6];
       const double gj2 = v[4] * v[4] + v[5] * v[5] + v[6] * v[6];
       e_elec[(size_t)w * d.N + k] = -0.5 * (v[3] + v[7] + 2.0 * cross + gj2);

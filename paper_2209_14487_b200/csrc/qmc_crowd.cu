@@ -888,7 +888,7 @@ int qmc_kinetic_energy(qmc_crowd_t* c, double* ekin_dev, double* e_elec_dev)
   if (c->state != ST_IDLE) return fail(QMC_ERR_STATE, "qmc_kinetic_energy in the middle of a move");
   if (!c->win_rows.empty()) return fail(QMC_ERR_STATE, "qmc_kinetic_energy needs a flushed window (call qmc_flush_delayed)");
   const CrowdDev& d = c->dev;
-  const size_t smem = (size_t)(3 * d.N + 32) * 8;
+  const size_t smem = (size_t)(3 * d.N) * 8;
   dim3 grid((d.N + EKIN_EPB - 1) / EKIN_EPB, d.W);
   {
     ProfScope ps(c, QMC_K_KINETIC);
