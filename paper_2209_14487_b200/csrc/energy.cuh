@@ -35,6 +35,7 @@ __global__ void __launch_bounds__(EKIN_NT) kinetic_kernel(CrowdDev d, double* __
     const T* cache = static_cast<const T*>(d.cache) + ((size_t)w * d.N + k) * 4 * ns;
     // v[0..2] = b.grad phi, v[3] = b.lap phi, v[4..6] = grad_k J, v[7] = lap_k J
     double v[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll 4   // 20 independent loads in flight per lane (the loop is otherwise one L2 round trip per iteration)
     for (int j = lane; j < d.M; j += 32) {
       const double bj = b[j];
       v[0] = fma(bj, (double)cache[j], v[0]);
@@ -43,6 +44,7 @@ __global__ void __launch_bounds__(EKIN_NT) kinetic_kernel(CrowdDev d, double* __
       v[3] = fma(bj, (double)cache[3 * ns + j], v[3]);
     }
     const double rk[3] = {R_s[3 * k], R_s[3 * k + 1], R_s[3 * k + 2]};
+#pragma unroll 2
     for (int i = lane; i < d.N; i += 32) {
       if (i == k) continue;
       double dd[3], r2 = 0.0;
