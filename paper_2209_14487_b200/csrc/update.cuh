@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d,
 #endif
 constexpr int FINTRI_NT = 128;
 template <int KDP>
-__global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize_tri_kernel(CrowdDev d)
+__global__ void __launch_bounds__(FINTRI_NT, KDP > 32 ? 2 : QMC_FINTRI_MIN_CTAS) flush_finalize_tri_kernel(CrowdDev d)
 {
   constexpr int KB = KDP / 8, SS = KDP + 1;
   extern __shared__ double s_n[];
@@ -374,7 +374,14 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
   for (int i = 0; i < 2; ++i)
 #pragma unroll
     for (int b = 0; b < KB; ++b) acc[i][b][0] = acc[i][b][1] = 0.0;
-  {
+  if (KB > 4) {
+    // eight window blocks: one fragment set at a time (two would spill next to the 64 accumulator registers)
+    Frag1<KB> fa;
+    for (int s = 0; s < ns; s += 16) {
+      load_frag1<KB>(fa, a0p, a1p, vp, s, ns, m, mb, g);
+      mma_frag1<KB>(acc, fa, mb);
+    }
+  } else {
     Frag1<KB> fa, fb;
     load_frag1<KB>(fa, a0p, a1p, vp, 0, ns, m, mb, g);
     for (int s = 0; s < ns; s += 32) {
@@ -400,7 +407,13 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
     }
   }
   // GEMM 2: B_strip = B0_strip + nw Z, 16 columns at a time
-  {
+  if (KB > 4) {
+    Frag2<KB> fa;
+    for (int j0 = ns - 16; j0 >= 0; j0 -= 16) {
+      load_frag2<KB>(fa, a0p, a1p, zp, j0, ns, m, mb, t);
+      mma_store_frag2<KB>(fa, acc, mb, a0p + j0, a1p + j0);
+    }
+  } else {
     // chunks in reverse order: the strip lines GEMM 1 read last are the most likely to still be in L2
     Frag2<KB> fa, fb;
     load_frag2<KB>(fa, a0p, a1p, zp, ns - 16, ns, m, mb, t);
