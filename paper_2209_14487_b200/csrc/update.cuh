@@ -182,17 +182,19 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d,
 #endif
 constexpr int FINTRI_NT = 128;
 template <int KDP>
-__global__ void __launch_bounds__(FINTRI_NT, KDP > 32 ? 2 : QMC_FINTRI_MIN_CTAS) flush_finalize_tri_kernel(CrowdDev d)
+__global__ void __launch_bounds__(FINTRI_NT, KDP > 32 ? 2 : QMC_FINTRI_MIN_CTAS) flush_finalize_tri_kernel(CrowdDev d, int l0)
 {
+  // l0 > 0: the window is flushed in sections of KDP accepted moves (section = moves l0 .. l0 + KDP - 1), each section a
+  // complete flush of its own applied to the result of the previous one (see launch_flush_kdp)
   constexpr int KB = KDP / 8, SS = KDP + 1;
   extern __shared__ double s_n[];
   const int w = blockIdx.x + d.w0;
-  const int m = d.mwin[w];
-  if (m == 0) return;
+  const int m = min(d.mwin[w] - l0, KDP);
+  if (m <= 0) return;
   const int ns = d.ns, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-  const double* Cp = d.Cp + (size_t)w * KDP * ns;
-  const double* V = d.V + (size_t)w * KDP * ns;
-  double* Z = d.C + (size_t)w * KDP * ns;
+  const double* Cp = d.Cp + ((size_t)w * d.kdp + l0) * ns;
+  const double* V = d.V + ((size_t)w * d.kdp + l0) * ns;
+  double* Z = d.C + ((size_t)w * d.kdp + l0) * ns;
   for (int e = tid; e < KDP * SS; e += FINTRI_NT) s_n[e] = 0.0;
   __syncthreads();
   for (int jb = warp; jb < KB && 8 * jb < m; jb += FINTRI_NT / 32) {
@@ -348,24 +350,24 @@ __device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double
 
 // Flush, step 2: B_strip <- B0_strip - (B0_strip V^T - E) Z.  KB = kdp / 8. grid = (ceil(ns / 64), W).
 template <int KB>
-__global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(CrowdDev d, int spin)
+__global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(CrowdDev d, int spin, int l0)
 {
   const int w = blockIdx.y + d.w0;
-  const int m = d.mwin[w];
-  if (m == 0) return;
+  const int m = min(d.mwin[w] - l0, 8 * KB);   // section l0 .. l0 + 8 KB - 1 of the window (l0 = 0: all of it)
+  if (m <= 0) return;
   const int ns = d.ns, kdp = d.kdp;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int row0 = (blockIdx.x * (FLUSH_NT / 32) + warp) * FLUSH_ROWS_PER_WARP;
   if (row0 >= ns) return;
   double* B = d.Binv + ((size_t)w * 2 + spin) * ns * ns;
-  const int* rows = d.rows + (size_t)w * kdp;
+  const int* rows = d.rows + (size_t)w * kdp + l0;
   const int mb = (m + 7) >> 3;  // 8-wide blocks of the window that hold accepted moves
   double* a0p = B + (size_t)(row0 + g) * ns + 4 * t;
   double* a1p = a0p + (size_t)8 * ns;
   // lane's V fragment base: row g of each window block, columns 4t..4t+3 of the chunk
-  const double* vp = d.V + (size_t)w * kdp * ns + (size_t)g * ns + 4 * t;
+  const double* vp = d.V + ((size_t)w * kdp + l0) * ns + (size_t)g * ns + 4 * t;
   // lane's Z fragment base: rows 2t (+q) of each window block, columns 2g, 2g+1 of the chunk
-  const double* zp = d.C + (size_t)w * kdp * ns + (size_t)(2 * t) * ns + 2 * g;
+  const double* zp = d.C + ((size_t)w * kdp + l0) * ns + (size_t)(2 * t) * ns + 2 * g;
 
   // GEMM 1: Wm = B0_strip V^T. acc[i][b] = tile (rows row0+8i.., window columns 8b..8b+7);
   // lane holds (row g, columns 8b+2t, 8b+2t+1).
