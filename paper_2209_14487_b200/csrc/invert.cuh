@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(INV_NT) invert_kernel(CrowdDev d)
 // Same elimination, same pivot choices, but right-looking in panels of INVB_NB columns so that the
 // matrix is swept 2 n / NB times instead of 2 n times (the unblocked kernel is bound by that
 // traffic: 3.7 TB at cfg 5 / W = 4096):
-//   (a) the panel (n x NB) is loaded into shared memory and eliminated there, unblocked, in place:
+//   (a) the panel (n x NB) is loaded into shared memory and eliminated there in place (in sub-panels of INVB_SB columns):
 //       afterwards it holds the NB columns X_G of the composite Gauss-Jordan operator G of the panel;
 //   (b) the panel's row swaps are applied to all other columns (column-local, no barrier);
 //   (c) the pivot rows A_K (NB x n) are copied to shared memory;
@@ -114,6 +114,7 @@ __global__ void __launch_bounds__(INV_NT) invert_kernel(CrowdDev d)
 //       32 x 32 register tiles per warp, fragments read conflict-free from padded shared memory.
 constexpr int INVB_NT = 512;
 constexpr int INVB_NB = 32;
+constexpr int INVB_SB = 8;            // sub-panel width inside the shared-memory panel
 constexpr int INVB_XS = INVB_NB + 4;   // row stride of the panel in smem (doubles): 4 g + t bank pattern
 
 inline __host__ __device__ size_t invert_blocked_smem(int ns)
@@ -133,7 +134,6 @@ __global__ void __launch_bounds__(INVB_NT) invert_blocked_kernel(CrowdDev d)
   double* redv = rowc + INVB_NB;
   int* redi = reinterpret_cast<int*>(redv + INVB_NT / 32);
   int* piv = redi + INVB_NT / 32;
-  __shared__ int s_p;
   __shared__ int s_bad;
   double* X = d.Binv + (size_t)blockIdx.x * ns * ns;
   if (tid == 0) s_bad = 0;
@@ -146,68 +146,126 @@ __global__ void __launch_bounds__(INVB_NT) invert_blocked_kernel(CrowdDev d)
       XG[r * INVB_XS + j] = (r < n && j < nb) ? X[(size_t)r * ns + c0 + j] : 0.0;
     }
     __syncthreads();
-    for (int j = 0; j < nb; ++j) {
-      const int c = c0 + j;
-      double best = -1.0;
-      int bi = c;
-      for (int r = c + tid; r < n; r += INVB_NT) {
-        double v = fabs(XG[r * INVB_XS + j]);
-        if (!(v == v)) v = INFINITY;
-        if (v > best) { best = v; bi = r; }
-      }
+    // The panel itself is eliminated in sub-panels of INVB_SB columns, the same right-looking scheme one level down:
+    // a pivot step touches n x SB elements (a warp takes four rows at a time, lane = (row, sub-panel column), the
+    // multiplier of a row is a shuffle, the row interchange is done on register copies of rows c and p, the search
+    // for the next pivot rides on the update), and after each sub-panel the other 32 - SB panel columns get its row
+    // swaps and one rank-SB update.  (Eliminating all 32 columns at every pivot step cost 67 of the kernel's 139 ms at
+    // cfg 5, W = 4096.)
+    constexpr int NW = INVB_NT / 32, SB = INVB_SB, RPW = 32 / SB;   // RPW rows per warp pass
+    static_assert(INVB_NB == 32 && SB == 8, "lane = panel column; four rows x eight columns per warp pass");
+    const int rsub = lane / SB, col = lane % SB, lbase = lane - col;
+    bool bad = false;
+    for (int s0 = 0; s0 < nb && !bad; s0 += SB) {
+      const int sb = min(SB, nb - s0);
+      {  // pivot candidates of the sub-panel's first column
+        double best = -1.0;
+        int bi = c0 + s0;
+        for (int r = c0 + s0 + tid; r < n; r += INVB_NT) {
+          double v = fabs(XG[r * INVB_XS + s0]);
+          if (!(v == v)) v = INFINITY;
+          if (v > best) { best = v; bi = r; }
+        }
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-        if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        for (int o = 16; o > 0; o >>= 1) {
+          const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+          const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+          if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if (lane == 0) { redv[warp] = best; redi[warp] = bi; }
       }
-      if (lane == 0) { redv[warp] = best; redi[warp] = bi; }
-      __syncthreads();
-      if (tid == 0) {
-        double bv = redv[0];
-        int bj = redi[0];
-        for (int q = 1; q < INVB_NT / 32; ++q)
-          if (redv[q] > bv || (redv[q] == bv && redi[q] < bj)) { bv = redv[q]; bj = redi[q]; }
-        s_p = bj;
-        piv[c] = bj;
-        if (!(bv > 0.0) || !isfinite(bv)) s_bad = 1;
+      for (int jl = 0; jl < sb; ++jl) {
+        const int c = c0 + s0 + jl;
+        __syncthreads();   // the partial maxima of this column (and the previous step's update) are complete
+        // every warp reduces the NW partial maxima itself: one shared-memory read per lane and a shuffle tree
+        static_assert(NW == 16, "the partial maxima fill half a warp");
+        double bv = redv[lane & (NW - 1)];
+        int p = redi[lane & (NW - 1)];
+#pragma unroll
+        for (int o = NW / 2; o > 0; o >>= 1) {
+          const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+          const int oi = __shfl_xor_sync(0xffffffffu, p, o);
+          if (ov > bv || (ov == bv && oi < p)) { bv = ov; p = oi; }
+        }
+        if (tid == 0) piv[c] = p;
+        if (!(bv > 0.0) || !isfinite(bv)) { bad = true; break; }   // uniform over the CTA
+        const double prow = XG[p * INVB_XS + s0 + col], crow = XG[c * INVB_XS + s0 + col];
+        const double pv = __shfl_sync(0xffffffffu, prow, lbase + jl);
+        const double rc = ((col == jl) ? 1.0 : prow) / pv;   // a true division (see above), one per lane
+        __syncthreads();   // rows c and p are in registers everywhere; the partial maxima have been read
+        double best = -1.0;
+        int bi = c + 1;
+        for (int rb = warp * RPW; rb < n; rb += 4 * RPW * NW) {   // warp-uniform trip count; four independent row groups
+          const int r0 = rb + rsub;
+          double v[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int r = r0 + i * RPW * NW;
+            v[i] = (r < n) ? XG[r * INVB_XS + s0 + col] : 0.0;
+            v[i] = (r == p) ? crow : v[i];   // row p receives the old row c
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int r = r0 + i * RPW * NW;
+            const double cf = __shfl_sync(0xffffffffu, v[i], lbase + jl);
+            double nv = fma(-cf, rc, (col == jl) ? 0.0 : v[i]);
+            nv = (r == c) ? rc : nv;
+            if (r < n) XG[r * INVB_XS + s0 + col] = nv;
+            double a = fabs(nv);
+            a = (a == a) ? a : INFINITY;
+            const bool take = r > c && r < n && (a > best || (a == best && r < bi));
+            best = take ? a : best;
+            bi = take ? r : bi;
+          }
+        }
+        if (jl + 1 < sb) {   // column jl + 1 lives in the lanes col == jl + 1 of the RPW row groups
+          double bj = __shfl_sync(0xffffffffu, best, lbase + jl + 1);
+          int ij = __shfl_sync(0xffffffffu, bi, lbase + jl + 1);
+#pragma unroll
+          for (int o = SB; o < 32; o <<= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, bj, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, ij, o);
+            if (ov > bj || (ov == bj && oi < ij)) { bj = ov; ij = oi; }
+          }
+          if (lane == 0) { redv[warp] = bj; redi[warp] = ij; }
+        }
       }
-      __syncthreads();
-      if (s_bad) break;
-      const int p = s_p;
-      if (p != c) {
-        if (tid < INVB_NB) {
-          const double a = XG[c * INVB_XS + tid], b = XG[p * INVB_XS + tid];
-          XG[c * INVB_XS + tid] = b;
-          XG[p * INVB_XS + tid] = a;
+      if (bad) break;
+      __syncthreads();   // the sub-panel holds its Gauss-Jordan operator; piv[] of its columns is visible
+      if (nb > sb) {
+        // the sub-panel's row swaps on the other panel columns (a thread owns a column: no barrier), then its pivot
+        // rows, then the rank-sb update X[:, o] <- X[:, o] + (G - E_K) A_K[:, o]  (rows of K: G[K, :] A_K[:, o])
+        double* AKs = AK;   // [SB][INVB_NB], free until step (c)
+        if (tid < INVB_NB && (tid < s0 || tid >= s0 + sb)) {
+          for (int q = 0; q < sb; ++q) {
+            const int c = c0 + s0 + q, p = piv[c];
+            if (p != c) {
+              const double x = XG[c * INVB_XS + tid], y = XG[p * INVB_XS + tid];
+              XG[c * INVB_XS + tid] = y;
+              XG[p * INVB_XS + tid] = x;
+            }
+          }
+          for (int q = 0; q < sb; ++q) AKs[q * INVB_NB + tid] = XG[(c0 + s0 + q) * INVB_XS + tid];
+        }
+        __syncthreads();
+        const bool other = lane < s0 || lane >= s0 + sb;   // lane = panel column again, a warp owns whole rows
+        double ak[SB];
+#pragma unroll
+        for (int q = 0; q < SB; ++q) ak[q] = (q < sb && other) ? AKs[q * INVB_NB + lane] : 0.0;
+#pragma unroll 2
+        for (int r = warp; r < n; r += NW) {
+          const double x = XG[r * INVB_XS + lane];
+          const bool in_k = r >= c0 + s0 && r < c0 + s0 + sb;
+          double acc = in_k ? 0.0 : x;
+#pragma unroll
+          for (int q = 0; q < SB; ++q) acc = fma(__shfl_sync(0xffffffffu, x, s0 + q), ak[q], acc);
+          if (other) XG[r * INVB_XS + lane] = acc;
         }
         __syncthreads();
       }
-      const double pv = XG[c * INVB_XS + j];
-      for (int r = tid; r < n; r += INVB_NT) colf[r] = XG[r * INVB_XS + j];
-      if (tid < nb) rowc[tid] = (tid == j) ? 1.0 / pv : XG[c * INVB_XS + tid] / pv;   // true divisions (see above)
-      __syncthreads();
-      if (nb == INVB_NB) {   // full panel: index arithmetic by shifts (an integer division per element otherwise)
-        static_assert((INVB_NB & (INVB_NB - 1)) == 0 && INVB_NT % INVB_NB == 0, "panel width must be a power of two");
-        const int jj = tid & (INVB_NB - 1);
-        const double rc = rowc[jj];
-        for (int r = tid / INVB_NB; r < n; r += INVB_NT / INVB_NB) {
-          double v;
-          if (r == c) v = rc;
-          else v = fma(-colf[r], rc, (jj == j) ? 0.0 : XG[r * INVB_XS + jj]);
-          XG[r * INVB_XS + jj] = v;
-        }
-      } else {
-        for (int e = tid; e < n * nb; e += INVB_NT) {
-          const int r = e / nb, jj = e - r * nb;
-          double v;
-          if (r == c) v = rowc[jj];
-          else v = fma(-colf[r], rowc[jj], (jj == j) ? 0.0 : XG[r * INVB_XS + jj]);
-          XG[r * INVB_XS + jj] = v;
-        }
-      }
-      __syncthreads();
     }
+    if (bad && tid == 0) s_bad = 1;
+    __syncthreads();
     if (s_bad) break;
     // (b) the panel's row swaps on every other column (a thread owns whole columns: no barrier needed)
     for (int o = tid; o < n; o += INVB_NT) {
