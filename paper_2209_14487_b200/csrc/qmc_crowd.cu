@@ -322,10 +322,10 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     // row over rho_l, whatever came before), and a section's Z solves only its own triangular block.  The strip kernel
     // with four window blocks keeps its double-buffered operands in registers (eight spill or lose the double
     // buffer): 11.1 -> 7.7 ms per flush of 64 moves at cfg 5, W = 4096.
-    for (int l0 = 0; l0 < KDP; l0 += 32) {
-      flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)32 * 33 * 8, st>>>(d, l0);
-      flush_kernel<4><<<grid, FLUSH_NT, 0, st>>>(d, spin, l0);
-    }
+    flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)32 * 33 * 8, st>>>(d, 0);
+    flush_kernel<4, 0><<<grid, FLUSH_NT, 0, st>>>(d, spin);
+    flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)32 * 33 * 8, st>>>(d, 32);
+    flush_kernel<4, 32><<<grid, FLUSH_NT, 0, st>>>(d, spin);
     return;
   }
   if (from_window) {
@@ -335,7 +335,7 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     dim3 fgrid((d.ns + fcols - 1) / fcols, wn);
     flush_finalize_kernel<KDP><<<fgrid, FINALIZE_NT, (size_t)KDP * KDP * 8, st>>>(d, spin);
   }
-  flush_kernel<KDP / 8><<<grid, FLUSH_NT, 0, st>>>(d, spin, 0);
+  flush_kernel<KDP / 8><<<grid, FLUSH_NT, 0, st>>>(d, spin);
 }
 
 // Flush of walkers [w0, w0 + wn) on stream st (the whole crowd on the crowd's stream by default).

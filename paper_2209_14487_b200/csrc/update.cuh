@@ -349,12 +349,21 @@ __device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double
 }
 
 // Flush, step 2: B_strip <- B0_strip - (B0_strip V^T - E) Z.  KB = kdp / 8. grid = (ceil(ns / 64), W).
-template <int KB>
-__global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(CrowdDev d, int spin, int l0)
+// L0: first move of the section this launch applies (-1: the whole window; a compile-time constant, so the common
+// case keeps the register allocation it was tuned with)
+template <int KB, int L0 = -1>
+__global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(CrowdDev d, int spin)
 {
+  constexpr int l0 = L0 < 0 ? 0 : L0;
   const int w = blockIdx.y + d.w0;
-  const int m = min(d.mwin[w] - l0, 8 * KB);   // section l0 .. l0 + 8 KB - 1 of the window (l0 = 0: all of it)
-  if (m <= 0) return;
+  // L0 < 0: the whole window; L0 >= 0: its section l0 .. l0 + 8 KB - 1
+  int m = d.mwin[w];
+  if constexpr (L0 < 0) {
+    if (m == 0) return;
+  } else {
+    m = min(m - l0, 8 * KB);
+    if (m <= 0) return;
+  }
   const int ns = d.ns, kdp = d.kdp;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int row0 = (blockIdx.x * (FLUSH_NT / 32) + warp) * FLUSH_ROWS_PER_WARP;
@@ -365,9 +374,9 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
   double* a0p = B + (size_t)(row0 + g) * ns + 4 * t;
   double* a1p = a0p + (size_t)8 * ns;
   // lane's V fragment base: row g of each window block, columns 4t..4t+3 of the chunk
-  const double* vp = d.V + ((size_t)w * kdp + l0) * ns + (size_t)g * ns + 4 * t;
+  const double* vp = d.V + (size_t)w * kdp * ns + (size_t)(g + l0) * ns + 4 * t;
   // lane's Z fragment base: rows 2t (+q) of each window block, columns 2g, 2g+1 of the chunk
-  const double* zp = d.C + ((size_t)w * kdp + l0) * ns + (size_t)(2 * t) * ns + 2 * g;
+  const double* zp = d.C + (size_t)w * kdp * ns + (size_t)(2 * t + l0) * ns + 2 * g;
 
   // GEMM 1: Wm = B0_strip V^T. acc[i][b] = tile (rows row0+8i.., window columns 8b..8b+7);
   // lane holds (row g, columns 8b+2t, 8b+2t+1).
