@@ -224,7 +224,13 @@ int rebuild(qmc_crowd* c)
   c->launches += 3;
   int st = c->is_f64 ? launch_build_t<double>(c) : launch_build_t<float>(c);
   if (st) return st;
-  const size_t bsmem = invert_blocked_smem(d.ns);
+  const size_t bsmem = invert_blocked_smem(d.ns), b2smem = invert_blocked2_smem(d.ns);
+#ifndef QMC_INVERT_V1
+  if (b2smem <= 227 * 1024 && d.ns <= 2 * INVB2_NT) {
+    if (b2smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_blocked2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b2smem));
+    invert_blocked2_kernel<<<(unsigned)(d.W * 2), INVB2_NT, b2smem, c->stream>>>(d);
+  } else
+#endif
   if (bsmem <= 227 * 1024 && d.ns <= INVB_NT) {
     if (bsmem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_blocked_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsmem));
     invert_blocked_kernel<<<(unsigned)(d.W * 2), INVB_NT, bsmem, c->stream>>>(d);
