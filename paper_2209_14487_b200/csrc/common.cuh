@@ -41,7 +41,8 @@ struct CrowdDev {
   double *V, *C, *Cp, *Sinv, *pvec, *yvec;
   int* rows;                                 // [W][kdp]
   int* mwin;                                 // [W]
-  double* e_elec;                            // [W][N] per-electron kinetic terms (qmc_kinetic_energy)
+  double* e_elec;                            // [W][N] per-electron kinetic terms (qmc_kinetic_energy); int[W N] build order
+  int* cell_bins;                            // [cells + 1] grid-cell histogram / offsets of the Slater build (or null)
   unsigned long long* counters;              // [0] accepted moves
   unsigned* sweep;                           // [1] Philox counter word 2
   int* status;                               // [1] != 0: singular matrix met
@@ -69,6 +70,16 @@ __device__ __forceinline__ void ld16_stream(const float* p, float (&v)[4], unsig
 __device__ __forceinline__ void ld16_stream(const double* p, double (&v)[2], unsigned long long pol)
 {
   asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v[0]), "=d"(v[1]) : "l"(p), "l"(pol));
+}
+// The same loads without the evict-first hint, for gathers that are arranged to re-use lines in L2 (spline_build_kernel
+// visits the positions in grid-cell order).
+__device__ __forceinline__ void ld16_keep(const float* p, float (&v)[4])
+{
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "l"(p));
+}
+__device__ __forceinline__ void ld16_keep(const double* p, double (&v)[2])
+{
+  asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v[0]), "=d"(v[1]) : "l"(p));
 }
 __device__ __forceinline__ void st16(float* p, const float (&v)[4])
 {

@@ -159,6 +159,8 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
   char* counters = take(4 * 8);
   char* sweep = take(4);
   char* status = take(4);
+  const size_t cells = (size_t)ds->grid[0] * ds->grid[1] * ds->grid[2];
+  char* cell_bins = cells <= ((size_t)1 << 22) ? take((cells + 1) * 4) : nullptr;   // Slater build in grid-cell order
   if (d) {
     d->R = (double*)R; d->Binv = (double*)Binv; d->cache = cache; d->vgl = vgl; d->brow = (double*)brow;
     d->rnew = (double*)rnew; d->delta = (double*)delta; d->g_old = (double*)g_old; d->g_new = (double*)g_new;
@@ -166,6 +168,7 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
     d->p = (double*)p; d->u = (double*)u; d->accepted = (unsigned char*)accepted;
     d->V = (double*)V; d->C = (double*)C; d->Cp = (double*)Cp; d->Sinv = (double*)Sinv; d->pvec = (double*)pvec; d->yvec = (double*)yvec;
     d->e_elec = (double*)e_elec;
+    d->cell_bins = (cells <= ((size_t)1 << 22)) ? (int*)cell_bins : nullptr;
     d->rows = (int*)rows; d->mwin = (int*)mwin; d->counters = (unsigned long long*)counters;
     d->sweep = (unsigned*)sweep; d->status = (int*)status;
     (void)acc_sink;
@@ -209,8 +212,28 @@ int launch_build_t(qmc_crowd* c)
   if (blocks > 0x7fffffffull) return fail(QMC_ERR_INVALID_ARG, "crowd too large for one build launch");
   const size_t smem = (size_t)5 * d.ns * sizeof(T);
   if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(spline_build_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  spline_build_kernel<T><<<(unsigned)blocks, SPLINE_NT, smem, c->stream>>>(d);
+  const int* order = nullptr;
+#ifndef QMC_BUILD_UNSORTED
+  if (d.cell_bins && blocks >= 256) {
+    // positions in grid-cell order (counting sort; the order inside a cell is arbitrary and does not matter: every
+    // CTA writes only its own electron's outputs).  The order lives in the e_elec scratch (W N doubles).
+    const int cells = d.grid[0] * d.grid[1] * d.grid[2];
+    int* ord = reinterpret_cast<int*>(d.e_elec);
+    CUDA_TRY(cudaMemsetAsync(d.cell_bins, 0, (size_t)(cells + 1) * 4, c->stream));
+    cell_count_kernel<<<(unsigned)((blocks + 255) / 256), 256, 0, c->stream>>>(d, d.cell_bins);
+    cell_scan_kernel<<<1, 1024, 0, c->stream>>>(d.cell_bins, cells);
+    cell_scatter_kernel<<<(unsigned)((blocks + 255) / 256), 256, 0, c->stream>>>(d, d.cell_bins, ord);
+    LAUNCH_CHECK(c);
+    c->launches += 3;
+    order = ord;
+  }
+#endif
+  spline_build_kernel<T><<<(unsigned)blocks, SPLINE_NT, smem, c->stream>>>(d, order);
   LAUNCH_CHECK(c);
+  if (order) {   // the sorted build writes A row-major: transpose to the A^T the inversion expects
+    transpose_inplace_kernel<<<dim3((unsigned)(d.ns / 16), (unsigned)(2 * d.W)), 256, 0, c->stream>>>(d);
+    LAUNCH_CHECK(c);
+  }
   return QMC_OK;
 }
 

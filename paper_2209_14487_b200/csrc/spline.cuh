@@ -69,7 +69,7 @@ __device__ __forceinline__ void spline_axis(const CrowdDev& d, int c, double x, 
 }
 
 // The 16 stencil rows (4 y x 4 z) of x-plane a for one 16-byte orbital slice `chunk`: 16 independent loads.
-template <typename T>
+template <typename T, bool KEEP = false>
 __device__ __forceinline__ void spline_plane_load(const T* __restrict__ tab, const SplineW<T>& s, int a, unsigned chunk,
                                                   T (&p)[4][4][Vec16<T>::W])
 {
@@ -80,7 +80,8 @@ __device__ __forceinline__ void spline_plane_load(const T* __restrict__ tab, con
   for (int b = 0; b < 4; ++b)
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
-      ld16_stream(tab + (size_t)(base + s.off[1][b] + s.off[2][c]) * VW, p[b][c], pol);
+      if (KEEP) ld16_keep(tab + (size_t)(base + s.off[1][b] + s.off[2][c]) * VW, p[b][c]);
+      else ld16_stream(tab + (size_t)(base + s.off[1][b] + s.off[2][c]) * VW, p[b][c], pol);
     }
 }
 
@@ -133,7 +134,8 @@ __device__ __forceinline__ double shfl_xor_t(double v, int m) { return __shfl_xo
 // their DRAM latency (a slot for work that is off the caller's critical path).
 struct NoSideWork { __device__ __forceinline__ void operator()(int) const {} };
 // r == nullptr: the caller has already filled `s` for this position (spline_axis per axis).
-template <typename T, int NT, typename Side = NoSideWork>
+// KEEP: loads without the L2 evict-first hint (callers that arrange for L2 re-use).
+template <typename T, int NT, typename Side = NoSideWork, bool KEEP = false>
 __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, SplineW<T>& s, T* vgl, Side side = Side())
 {
   constexpr int VW = Vec16<T>::W;
@@ -151,7 +153,7 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
     T out[5][VW];
     if (chunk < d.tab_vecs && chunk < chunks) {
       T p[4][4][VW];
-      spline_plane_load<T>(tab, s, a, chunk, p);
+      spline_plane_load<T, KEEP>(tab, s, a, chunk, p);
       if (c0 == 0 && tid >= 32) side(tid);
       spline_plane_sum<T>(s, a, p, out);
     } else {
@@ -207,21 +209,95 @@ __global__ void __launch_bounds__(SPLINE_NT, 4) spline_vgl_kernel(CrowdDev d)
 // qmc_crowd_create / set_positions: one CTA per (walker, electron) at the electron's own position;
 // fills the caches and the transposed Slater matrix X[j][i] = phi_j(r_i) that the inversion kernel
 // turns into B = (A^-1)^T = (A^T)^-1 (D:C2).  dynamic smem: 5 ns elements of T.
+// order != nullptr: CTA b takes (walker, electron) order[b] -- the positions sorted by grid cell (below), so that CTAs
+// in flight together gather overlapping stencils and the table is streamed from DRAM about once instead of once per
+// position (308 GB at cfg 5, W = 4096); the loads then keep their lines in L2.  CTAs of one walker are then no longer
+// neighbours in time, so the Slater matrix is written row-major (A, one contiguous row per electron: the strided
+// 8-byte writes of A^T would stop merging in L2) and transposed in place afterwards (transpose_inplace_kernel).
 template <typename T>
-__global__ void __launch_bounds__(SPLINE_NT, 4) spline_build_kernel(CrowdDev d)
+__global__ void __launch_bounds__(SPLINE_NT, 4) spline_build_kernel(CrowdDev d, const int* __restrict__ order)
 {
   extern __shared__ double sm_build[];
   __shared__ SplineW<T> s;
   T* v_s = reinterpret_cast<T*>(sm_build);
-  const size_t we = blockIdx.x;
+  const size_t we = order ? (size_t)order[blockIdx.x] : (size_t)blockIdx.x;
   const int w = (int)(we / d.N), e_idx = (int)(we - (size_t)w * d.N);
-  spline_cta<T, SPLINE_NT>(d, d.R + 3 * we, s, v_s);
+  if (order) spline_cta<T, SPLINE_NT, NoSideWork, true>(d, d.R + 3 * we, s, v_s);
+  else spline_cta<T, SPLINE_NT>(d, d.R + 3 * we, s, v_s);
   __syncthreads();
   const int spin = e_idx / d.n, i = e_idx - spin * d.n;
   T* cache = static_cast<T*>(d.cache) + we * 4 * d.ns;
   double* X = d.Binv + ((size_t)w * 2 + spin) * d.ns * d.ns;
   for (int j = threadIdx.x; j < 4 * d.ns; j += SPLINE_NT) cache[j] = v_s[d.ns + j];
-  for (int j = threadIdx.x; j < d.M; j += SPLINE_NT) X[(size_t)j * d.ns + i] = (double)v_s[j];
+  if (order) {
+    for (int j = threadIdx.x; j < d.M; j += SPLINE_NT) X[(size_t)i * d.ns + j] = (double)v_s[j];
+  } else {
+    for (int j = threadIdx.x; j < d.M; j += SPLINE_NT) X[(size_t)j * d.ns + i] = (double)v_s[j];
+  }
+}
+
+// X <- X^T for every ns x ns matrix of the crowd, in place: CTA (a, matrix) swaps the 16 x 16 tiles (a, b) and (b, a)
+// for b >= a through shared memory (coalesced both ways).  grid = (ns / 16, 2 W), 256 threads.
+__global__ void __launch_bounds__(256) transpose_inplace_kernel(CrowdDev d)
+{
+  __shared__ double t0[16][17], t1[16][17];
+  const int ns = d.ns, a = blockIdx.x, tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  double* X = d.Binv + (size_t)blockIdx.y * ns * ns;
+  for (int b = a; b < ns / 16; ++b) {
+    t0[ty][tx] = X[(size_t)(16 * a + ty) * ns + 16 * b + tx];
+    t1[ty][tx] = X[(size_t)(16 * b + ty) * ns + 16 * a + tx];
+    __syncthreads();
+    X[(size_t)(16 * b + ty) * ns + 16 * a + tx] = t0[tx][ty];
+    if (b != a) X[(size_t)(16 * a + ty) * ns + 16 * b + tx] = t1[tx][ty];
+    __syncthreads();
+  }
+}
+
+// ---- counting sort of the (walker, electron) positions by grid cell, z fastest like the table ----------------------
+__device__ __forceinline__ int cell_of(const CrowdDev& d, const double* r)
+{
+  int idx = 0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    double u = r[c] * d.inv_box[c];
+    u -= floor(u);
+    int i = (int)(u * d.grid[c]);
+    i = i < 0 ? 0 : (i >= d.grid[c] ? d.grid[c] - 1 : i);   // non-finite positions land in the first / last cell
+    idx = idx * d.grid[c] + i;
+  }
+  return idx;
+}
+__global__ void cell_count_kernel(CrowdDev d, int* bins)
+{
+  const size_t we = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (we < (size_t)d.W * d.N) atomicAdd(bins + cell_of(d, d.R + 3 * we), 1);
+}
+// exclusive scan of bins[0 .. nb) in place, one CTA of 1024 threads, each thread a contiguous chunk
+__global__ void __launch_bounds__(1024) cell_scan_kernel(int* bins, int nb)
+{
+  __shared__ int part[1024];
+  const int tid = threadIdx.x, per = (nb + 1023) / 1024, lo = min(tid * per, nb), hi = min(lo + per, nb);
+  int sum = 0;
+  for (int i = lo; i < hi; ++i) sum += bins[i];
+  part[tid] = sum;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const int v = tid >= o ? part[tid - o] : 0;
+    __syncthreads();
+    part[tid] += v;
+    __syncthreads();
+  }
+  int run = part[tid] - sum;
+  for (int i = lo; i < hi; ++i) {
+    const int v = bins[i];
+    bins[i] = run;
+    run += v;
+  }
+}
+__global__ void cell_scatter_kernel(CrowdDev d, int* bins, int* order)
+{
+  const size_t we = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (we < (size_t)d.W * d.N) order[atomicAdd(bins + cell_of(d, d.R + 3 * we), 1)] = (int)we;
 }
 
 }  // namespace qmc
