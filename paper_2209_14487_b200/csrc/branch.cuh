@@ -104,4 +104,20 @@ __global__ void slots_check_kernel(CrowdDev d, int n, const int* __restrict__ sl
   if (atomicAdd(marks + w, 1) != 0) atomicOr(d.status, 8);
 }
 
+// CTAs per walker of the state copies: about 32 16-byte vectors per thread
+inline int state_chunks(const WalkerState& ws)
+{
+  const size_t vecs = ws.total() / 16;
+  int chunks = (int)((vecs + (size_t)BRANCH_NT * 32 - 1) / ((size_t)BRANCH_NT * 32));
+  return chunks < 1 ? 1 : (chunks > 64 ? 64 : chunks);
+}
+
+// *out += number of slots with src[w] != w
+__global__ void branch_count_kernel(int W, const int* __restrict__ src, int* out)
+{
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned b = __ballot_sync(0xffffffffu, w < W && src[w] != w);
+  if ((threadIdx.x & 31) == 0 && b) atomicAdd(out, __popc(b));
+}
+
 }  // namespace qmc

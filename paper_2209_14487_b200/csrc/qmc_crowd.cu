@@ -948,21 +948,6 @@ int qmc_kinetic_energy(qmc_crowd_t* c, double* ekin_dev, double* e_elec_dev)
   return QMC_OK;
 }
 
-// CTAs per walker of the state copies: about 32 16-byte vectors per thread
-int state_chunks(const WalkerState& ws)
-{
-  const size_t vecs = ws.total() / 16;
-  int chunks = (int)((vecs + (size_t)BRANCH_NT * 32 - 1) / ((size_t)BRANCH_NT * 32));
-  return chunks < 1 ? 1 : (chunks > 64 ? 64 : chunks);
-}
-
-__global__ void branch_count_kernel(int W, const int* __restrict__ src, int* out)
-{
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
-  const unsigned b = __ballot_sync(0xffffffffu, w < W && src[w] != w);
-  if ((threadIdx.x & 31) == 0 && b) atomicAdd(out, __popc(b));
-}
-
 int qmc_crowd_branch(qmc_crowd_t* c, const int32_t* src_dev, int* n_copied)
 {
   if (!c || !src_dev) return fail(QMC_ERR_INVALID_ARG, "NULL argument");
