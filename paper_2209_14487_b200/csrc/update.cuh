@@ -204,6 +204,7 @@ __global__ void __launch_bounds__(FINTRI_NT, KDP > 32 ? 2 : QMC_FINTRI_MIN_CTAS)
     const bool a_ok = 8 * jb + g < m;
     const double* ap = Cp + (size_t)(8 * jb + g) * ns + 4 * t;
     const double* vp = V + (size_t)g * ns + 4 * t;
+#pragma unroll 2   // two chunks of fragment loads in flight (the loop is a chain of L2 round trips otherwise)
     for (int s = 0; s < ns; s += 16) {
       double a[4] = {0.0, 0.0, 0.0, 0.0};
       if (a_ok) ld32(ap + s, a);
