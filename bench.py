@@ -288,7 +288,7 @@ def time_multi_crowd(wl, W, C, kd, coefs_dev, dev, steps=2, warmup=1):
     return e0.elapsed_time(e1), prop, acc
 
 
-def drift_study(wl, coefs_dev, dev, W=128, ranks=(1, 32, 64), marks=(1, 5, 10, 20, 50, 100)):
+def drift_study(wl, coefs_dev, dev, W=128, ranks=(1, 32, 64), marks=(1, 5, 10, 20, 50, 100), fp32_round=False):
     """Round-off drift of the carried inverses: after S free-running sweeps, the largest and
     median norm-wise difference between a walker's carried inverse and the one recomputed at the same positions."""
     import torch
@@ -299,7 +299,13 @@ def drift_study(wl, coefs_dev, dev, W=128, ranks=(1, 32, 64), marks=(1, 5, 10, 2
         c, f = mk(), mk()
         done = 0
         for S in marks:
-            c.qmc_sweep(S - done)
+            if fp32_round:   # a lower bound on what an fp32-stored inverse would do: round after every sweep
+                for _ in range(S - done):
+                    c.qmc_sweep(1)
+                    for spin in (0, 1):
+                        c.set_inverse(spin, c.inverse(spin).float().double())
+            else:
+                c.qmc_sweep(S - done)
             done = S
             f.set_positions(c.positions())
             worst, med = 0.0, 0.0
@@ -307,8 +313,8 @@ def drift_study(wl, coefs_dev, dev, W=128, ranks=(1, 32, 64), marks=(1, 5, 10, 2
                 B, F = c.inverse(spin), f.inverse(spin)
                 rel = (B - F).abs().amax(dim=(1, 2)) / F.abs().amax(dim=(1, 2))
                 worst, med = max(worst, float(rel.max())), max(med, float(rel.median()))
-            print(json.dumps({"drift": True, "walkers": W, "delay_rank": kd, "sweeps": S, "rel_diff_max": worst,
-                              "rel_diff_median": med}), flush=True)
+            print(json.dumps({"drift": True, "fp32_rounded_every_sweep": fp32_round, "walkers": W, "delay_rank": kd,
+                              "sweeps": S, "rel_diff_max": worst, "rel_diff_median": med}), flush=True)
         c.close()
         f.close()
 
@@ -541,6 +547,7 @@ def run_cuda(args):
                 torch.cuda.empty_cache()
     if args.drift and world == 1:
         drift_study(wl, coefs_dev, dev)
+        drift_study(wl, coefs_dev, dev, ranks=(32,), marks=(1, 2, 5, 10, 20), fp32_round=True)
     if args.multi_crowd and world == 1:
         # S:8(f) item 1: does splitting a crowd of W into C crowds on C streams / host threads pay at small W?
         for W2 in (256, 512, 1024, 4096):
