@@ -206,6 +206,28 @@ __device__ __forceinline__ void warp_sum8(double (&v)[8])
   for (int q = 0; q < 8; ++q) v[q] = __shfl_sync(0xffffffffu, e, ((q >> 2) & 1) * 16 + ((q >> 1) & 1) * 8 + (q & 1) * 4);
 }
 
+// 1/x and 1/sqrt(x) for normal positive x: the hardware's approximate seed (MUFU.RCP64H / RSQ64H, ~2^-23) and two Newton
+// steps in fma arithmetic (~2^-46, then full double precision to within an ulp or two), without the special-case
+// branches of the library versions.  Used by the Jastrow pair terms, whose arguments are well inside the normal range.
+__device__ __forceinline__ double rcp_pos(double x)
+{
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ double rsqrt_pos(double x)
+{
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-(x * y), 0.5 * y, 0.5);
+  y = fma(y, e, y);
+  e = fma(-(x * y), 0.5 * y, 0.5);
+  return fma(y, e, y);
+}
+
 // ---- Philox4x32-10 (Salmon et al., SC'11; D:C7). Counter (walker id, k, sweep, tag). ----
 __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0,
                                               unsigned k1, unsigned (&out)[4])

@@ -55,10 +55,10 @@ __global__ void __launch_bounds__(EKIN_NT) kinetic_kernel(CrowdDev d, double* __
         dd[c] = x;
         r2 = fma(x, x, r2);
       }
-      if (r2 > 0.0) {
-        const double inv_r = rsqrt(r2);
+      if (r2 > 1e-280) {   // as j2_pair (move.cuh)
+        const double inv_r = rsqrt_pos(r2);
         const double r = r2 * inv_r;
-        const double inv_den = 1.0 / fma(d.j2_b, r, 1.0);
+        const double inv_den = rcp_pos(fma(d.j2_b, r, 1.0));
         const double du = d.j2_a * inv_den * inv_den;
         const double f = du * inv_r;
 #pragma unroll

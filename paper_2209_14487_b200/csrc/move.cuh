@@ -59,10 +59,10 @@ __device__ __forceinline__ void j2_pair(const CrowdDev& d, const double (&rk)[3]
     dd[c] = x;
     r2 = fma(x, x, r2);
   }
-  if (r2 > 0.0) {
-    const double inv_r = rsqrt(r2);
+  if (r2 > 1e-280) {   // coincident electrons contribute nothing (D:C3); anything else is far inside the normal range
+    const double inv_r = rsqrt_pos(r2);
     const double r = r2 * inv_r;
-    const double inv_den = 1.0 / fma(d.j2_b, r, 1.0);
+    const double inv_den = rcp_pos(fma(d.j2_b, r, 1.0));
     usum += d.j2_a * r * inv_den;
     const double f = d.j2_a * inv_den * inv_den * inv_r;
 #pragma unroll
