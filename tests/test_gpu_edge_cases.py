@@ -83,3 +83,21 @@ def test_argument_and_state_errors():
     with pytest.raises(q.QmcError) as e:              # odd electron count
         q.Crowd(torch.from_numpy(coefs).cuda(), wl.box, torch.from_numpy(pos[:, :7].copy()).cuda(), tau=0.01)
     assert e.value.status == q.QMC_ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("tau,kd", [(1e-6, 8), (1e-6, 1), (0.6, 8), (0.6, 1), (0.6, 32)])
+def test_acceptance_extremes(tau, kd):
+    """Nearly every move accepted (full windows, m = k) and nearly every move rejected (windows with m = 0 or 1, flushes
+    that have nothing to do): the free-running trajectory still equals the oracle's on an fp64 table."""
+    wl = qi.small_workload(n_elec=80, grid=12, box=7.0, coef_dtype="f64", coef_dist="uniform", n_walkers=5, tau=tau,
+                           delay_rank=kd, cfg=76)
+    crowd, osys, _, pos = make_pair(wl)
+    oc = oracle.OracleCrowd(osys, pos)
+    acc = oc.sweep(2)
+    crowd.qmc_sweep(2)
+    frac = acc / (2 * 5 * 80)
+    assert frac > 0.98 if tau < 1e-3 else frac < 0.5, frac
+    assert crowd.stats()["accepted"] == acc
+    assert np.array_equal(npy(crowd.positions()), oc.positions())
+    for spin in (0, 1):
+        assert relerr(npy(crowd.inverse(spin)), oc.inverse(spin)) < 1e-10
