@@ -101,3 +101,30 @@ def test_acceptance_extremes(tau, kd):
     assert np.array_equal(npy(crowd.positions()), oc.positions())
     for spin in (0, 1):
         assert relerr(npy(crowd.inverse(spin)), oc.inverse(spin)) < 1e-10
+
+
+@pytest.mark.parametrize("kd", [1, 8])
+def test_anisotropic_grid_and_box(kd):
+    """Different grid sizes and box lengths per axis (the C ABI takes grid[3], box[3]): a transposed axis anywhere in the
+    stencil offsets, the weights or the minimum image would move the trajectory off the oracle's."""
+    import torch
+    import paper_2209_14487_b200 as q
+    n_elec, W, grid, box = 24, 4, (6, 9, 11), (3.0, 4.5, 5.5)
+    rng = np.random.default_rng(77)
+    coefs = rng.uniform(-1.0, 1.0, size=grid + (n_elec // 2,))
+    pos = rng.uniform(0.0, 1.0, size=(W, n_elec, 3)) * np.array(box)
+    osys = oracle.OracleSystem(n_elec, grid, box, coefs, j2_a=0.5, j2_b=1.0, tau=0.02, seed=5, delay_rank=kd)
+    oc = oracle.OracleCrowd(osys, pos)
+    crowd = q.Crowd(torch.from_numpy(coefs).cuda(), box, torch.from_numpy(pos).cuda(), tau=0.02, delay_rank=kd,
+                    j2_a=0.5, j2_b=1.0, seed=5)
+    acc = oc.sweep(3)
+    crowd.qmc_sweep(3)
+    assert crowd.stats()["accepted"] == acc
+    assert np.array_equal(npy(crowd.positions()), oc.positions())
+    for spin in (0, 1):
+        assert relerr(npy(crowd.inverse(spin)), oc.inverse(spin)) < 1e-10
+    phi, dphi, d2phi = (npy(x) for x in crowd.qmc_spo_vgl(0, want_outputs=True))
+    mv = npy(crowd.move()["rnew"])
+    for w in range(W):
+        p, dp, d2p = osys.spo_vgl(mv[w])
+        assert relerr(phi[w], p) < 1e-12 and relerr(dphi[w], dp) < 1e-12 and relerr(d2phi[w], d2p) < 1e-12
