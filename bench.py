@@ -52,22 +52,33 @@ def parse_args():
                     help="also print the drift of the carried inverses against a recompute after 1..100 sweeps")
     ap.add_argument("--no-probes", action="store_true", help="skip the step-call / rank-1 kernel probes")
     ap.add_argument("--ref-walkers", type=int, default=None, help="walkers of the oracle sample (default = cores)")
+    ap.add_argument("--no-sweep-points", action="store_true",
+                    help="skip the compact crowd-size / delay-rank sweep carried inside the JSON line")
+    ap.add_argument("--plan-only", action="store_true",
+                    help="no GPU work: every rank reports its walker range (gloo), rank 0 prints the plan as JSON")
     return ap.parse_args()
+
+
+# FP64 DMMA issue ceiling of one B200: 148 SMs x 64 FMA/clk/SM x 2 flop x 1.965 GHz (guide unit counts and max SM clock;
+# a bare DMMA.8x8x4 loop measured exactly this in round 1, update.cuh).  The flush runs at the full SM clock (the
+# bf16 "sustained" figure of MEASURED_PEAKS.json is power-capped at ~1.3 GHz and does not describe it).
+FP64_DMMA_CEILING_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 
 def peaks():
     """Roofline denominators: MEASURED_PEAKS.json (driver-written) or the profiling guide's fallback.
-    FP64 tensor: no measured entry exists, so it is the measured bf16 GEMM peak x the guide's nominal
-    ratio 45 / 2250 (sustained figure: the flush is timed inside a long step)."""
+    FP64 tensor: MEASURED_PEAKS.json has no entry.  The denominator of the flush is the larger of the cuBLAS DGEMM
+    probe of the same run and the DMMA issue ceiling (filled in by run_cuda); the guide-derived figure (measured
+    sustained bf16 GEMM x nominal 45/2250) is kept beside it for reference only -- it is lower than what cuBLAS
+    reaches on the same box."""
     p = ROOT / "MEASURED_PEAKS.json"
     if p.exists():
         d = json.loads(p.read_text())
         bf16 = float(d.get("bf16_tflops_sustained", d.get("bf16_tflops", 1400.0)))
-        return {"hbm_gbs": float(d["hbm_gbs"]), "fp64_tflops": bf16 * 45.0 / 2250.0,
-                "source": "measured (MEASURED_PEAKS.json)",
-                "fp64_source": "measured sustained bf16 GEMM x nominal 45/2250"}
-    return {"hbm_gbs": 6650.0, "fp64_tflops": 1400.0 * 45.0 / 2250.0, "source": "fallback (B200_PROFILING.md)",
-            "fp64_source": "fallback sustained bf16 1.4 PF x nominal 45/2250"}
+        return {"hbm_gbs": float(d["hbm_gbs"]), "fp64_bf16_derived_tflops": bf16 * 45.0 / 2250.0,
+                "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "fp64_bf16_derived_tflops": 1400.0 * 45.0 / 2250.0,
+            "source": "fallback (B200_PROFILING.md)"}
 
 
 class ClockSampler:
@@ -189,14 +200,18 @@ def algorithmic(wl, W, kd, alpha, el, m_move=None):
         "ratio_grad": {"bytes": ratio_b},
         "accept": {"bytes": accept_b},
         "ratio_accept": {"bytes": ratio_b + accept_b},
-        # fused ratio(k) + accept(k) + row(k+1): C rows and positions are needed once, not twice
-        "fused_move": {"bytes": ratio_b + accept_b + row_b - alpha * W * 8 * n * m_move - W * 24 * N},
         # one launch = all kd moves of a delay window in the eager-block form (window.cuh): per move the
         # spline gather, one inverse row and one gradient-cache row; per accepted move the cache / V / Cp
         # rows written and the still-to-be-proposed rows of the block read and rewritten ((kd-1)/2 on average);
         # positions once per window.  Orbitals at r' never leave the SM.
-        "window": {"bytes": W * (kd * (64 * M * el + 8 * n + 3 * M * el)
-                                 + alpha * kd * (4 * M * el + 16 * n + 16 * n * (kd - 1) / 2) + 24 * N),
+        # "bytes" = the COMPULSORY HBM bytes of that launch: the gather (table >> L2), the first touch of the block's
+        # kd rows and the write-back of their final values, the gradient-cache rows read and (accepted) written, the
+        # V / Cp rows written for the flush, positions.  The block rows a walker re-reads and re-writes inside its own
+        # window (16 n (kd-1)/2 per accepted move) are L2-resident by construction (98 KB per walker x 592 resident
+        # walkers) and are counted only in "l2_plus_hbm_bytes".
+        "window": {"bytes": W * (kd * (64 * M * el + 3 * M * el + 16 * n) + alpha * kd * (4 * M * el + 16 * n) + 24 * N),
+                   "l2_plus_hbm_bytes": W * (kd * (64 * M * el + 8 * n + 3 * M * el)
+                                             + alpha * kd * (4 * M * el + 16 * n + 16 * n * (kd - 1) / 2) + 24 * N),
                    "flops": kd * W * 600 * M},
         # kinetic energy: both inverses, the four cache rows of every electron, positions; ~30 fp64 flop per pair term
         # (min image, rsqrt, reciprocal, u', u'') and 8 per (electron, orbital) of the four dots
@@ -319,17 +334,35 @@ def drift_study(wl, coefs_dev, dev, W=128, ranks=(1, 32, 64), marks=(1, 5, 10, 2
         f.close()
 
 
+def csrc_digest():
+    """sha256 (first 16 hex digits) over the CUDA sources and the C header: names the kernels a capture was made with
+    (the GPU box has no .git, so a commit id cannot be read there)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted((ROOT / "paper_2209_14487_b200" / "csrc").glob("*.cu*")) + [ROOT / "include" / "qmc_crowd.h"]:
+        h.update(f.name.encode())
+        h.update(f.read_bytes())
+    return h.hexdigest()[:16]
+
+
 def ncu_traffic(cfg, W, kd):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu captures
-    (profiles/r1_dram_traffic.csv: cfg,walkers,delay_rank,kernel,bytes), for the configuration timed here."""
-    out = {}
-    f = ROOT / "profiles" / "r1_dram_traffic.csv"
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
+    (profiles/dram_traffic.csv: cfg,walkers,delay_rank,kernel,bytes,csrc_digest), for the configuration timed here.
+    Returns ({kernel: bytes}, source): an entry is used only if it was captured with the kernel sources that are being
+    timed now (same csrc_digest); otherwise the field is null -- a stale capture is not a measurement of this run."""
+    out, src = {}, None
+    f = ROOT / "profiles" / "dram_traffic.csv"
     if f.exists():
+        now = csrc_digest()
         for ln in f.read_text().splitlines():
             c = [x.strip() for x in ln.split(",")]
-            if len(c) == 5 and c[0].isdigit() and (int(c[0]), int(c[1]), int(c[2])) == (cfg, W, kd):
-                out[c[3]] = float(c[4])
-    return out
+            if len(c) == 6 and c[0].isdigit() and (int(c[0]), int(c[1]), int(c[2])) == (cfg, W, kd):
+                if c[5] == now:
+                    out[c[3]] = float(c[4])
+                    src = f"profiles/dram_traffic.csv @ csrc {now}"
+                elif src is None:
+                    src = f"stale: profiles/dram_traffic.csv was captured at csrc {c[5]}, timed sources are {now}"
+    return out, src
 
 
 def fp64_probe():
@@ -427,11 +460,33 @@ def run_cuda(args):
         ent["hbm_frac"] = ent["gbs"] / pk["hbm_gbs"]
         kernels[name] = ent
     dom = max(kernels, key=lambda k: kernels[k]["share"])
-    traffic = ncu_traffic(args.cfg, W, kd)
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "frac": kernels[dom]["gbs"] / pk["hbm_gbs"], "traffic": traffic.get(dom), "peak_source": pk["source"],
-                "share_of_step": kernels[dom]["share"],
-                "algorithmic_bytes_per_launch": alg[dom]["bytes"]}
+    traffic, traffic_source = ncu_traffic(args.cfg, W, kd)
+
+    def with_traffic(ent, name):
+        """traffic = ncu dram bytes per launch (null unless captured with the sources timed now); dram_frac = that
+        traffic over the event-timed duration of this run over the measured copy rate."""
+        t = traffic.get(name)
+        ent["traffic"] = t
+        ent["traffic_source"] = traffic_source
+        if t and ent.get("avg_us"):
+            ent["dram_frac"] = t / (ent["avg_us"] * 1e-6) / 1e9 / pk["hbm_gbs"]
+        return ent
+
+    roofline = with_traffic({"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["gbs"], "peak": pk["hbm_gbs"],
+                             "unit": "GB/s", "frac": kernels[dom]["gbs"] / pk["hbm_gbs"],
+                             "peak_source": pk["source"] + ", of measured", "share_of_step": kernels[dom]["share"],
+                             "avg_us": kernels[dom]["avg_us"], "algorithmic_bytes_per_launch": alg[dom]["bytes"],
+                             "bytes_counted": "compulsory HBM bytes (DESIGN.md section 6)"}, dom)
+    if "l2_plus_hbm_bytes" in alg[dom]:
+        # the round-1 figure: every byte the kernel requests beyond L1, including the block rows that stay in L2
+        roofline["l2_plus_hbm_bytes"] = alg[dom]["l2_plus_hbm_bytes"]
+        roofline["l2_plus_hbm_gbs"] = alg[dom]["l2_plus_hbm_bytes"] / (kernels[dom]["avg_us"] * 1e-6) / 1e9
+    probe, probe_err = None, None
+    if rank == 0:
+        try:
+            probe = fp64_probe()
+        except Exception as e:  # probe only
+            probe_err = str(e)[:80]
     extra_rooflines = {}
     if "flush" in kernels:
         n = wl.n
@@ -440,29 +495,38 @@ def run_cuda(args):
         while kdp < kd:
             kdp *= 2
         executed = useful * (4 * n * n * kdp + 2 * n * kdp * kdp) / max(alg["flush"]["flops"] / W, 1.0)
-        extra_rooflines["flush"] = {
-            "kernel": "flush (finalize + DMMA strip)", "bound": "tensor", "achieved": useful, "peak": pk["fp64_tflops"],
-            "unit": "TFLOP/s", "frac": useful / pk["fp64_tflops"], "traffic": traffic.get("flush"),
-            "peak_source": pk["fp64_source"], "share_of_step": kernels["flush"]["share"],
-            "executed_tflops_with_padding": executed, "hbm_frac": kernels["flush"]["hbm_frac"]}
+        # denominator: whichever is larger of what cuBLAS DGEMM reaches in this run and the DMMA issue ceiling
+        peak64 = max(probe or 0.0, FP64_DMMA_CEILING_TFLOPS)
+        extra_rooflines["flush"] = with_traffic({
+            "kernel": "flush (finalize + DMMA strip)", "bound": "tensor", "achieved": useful, "peak": peak64,
+            "unit": "TFLOP/s", "frac": useful / peak64,
+            "peak_source": "max(cuBLAS DGEMM 8192^3 probe of this run, DMMA issue ceiling 148 SM x 64 FMA/clk x 1.965 GHz)",
+            "share_of_step": kernels["flush"]["share"], "avg_us": kernels["flush"]["avg_us"],
+            "executed_tflops_with_padding": executed, "executed_frac": executed / peak64,
+            "frac_of_dgemm_probe": (useful / probe) if probe else None,
+            "frac_of_dmma_issue_ceiling": useful / FP64_DMMA_CEILING_TFLOPS,
+            "frac_of_bf16_derived_peak": useful / pk["fp64_bf16_derived_tflops"],
+            "bf16_derived_peak_tflops": pk["fp64_bf16_derived_tflops"],
+            "hbm_frac": kernels["flush"]["hbm_frac"]}, "flush")
     if "kinetic" in kernels:
         # plain fp64 ALU work (J2 pair terms): peak = 148 SMs x 64 FMA/clk x 2 x max SM clock
         k_ = kernels["kinetic"]
         tf = alg["kinetic"]["flops"] / (k_["avg_us"] * 1e-6) / 1e12
-        alu_peak = 148 * 64 * 2 * 1.965e9 / 1e12
+        alu_peak = FP64_DMMA_CEILING_TFLOPS
         extra_rooflines["kinetic"] = {"kernel": "kinetic_kernel (qmc_kinetic_energy)", "bound": "alu", "achieved": tf,
                                       "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak, "traffic": None,
                                       "avg_us": k_["avg_us"], "hbm_frac": k_["hbm_frac"]}
     for name in ("spline_vgl", "rank1", "branch"):
         if name in kernels:
-            extra_rooflines[name] = {"kernel": name, "bound": "hbm", "achieved": kernels[name]["gbs"],
-                                     "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": kernels[name]["hbm_frac"],
-                                     "traffic": traffic.get(name), "share_of_step": kernels[name]["share"]}
+            extra_rooflines[name] = with_traffic({"kernel": name, "bound": "hbm", "achieved": kernels[name]["gbs"],
+                                                  "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": kernels[name]["hbm_frac"],
+                                                  "avg_us": kernels[name]["avg_us"],
+                                                  "share_of_step": kernels[name]["share"]}, name)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64" if kd else "f64", "data": "synthetic",
+        "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"cfg{args.cfg}_{wl.n_elec}e_k{kd}", "walkers_per_gpu": W, "n_elec": wl.n_elec,
                    "grid": wl.grid, "table_dtype": wl.coef_dtype, "delay_rank": kd, "sweeps_per_step": 1,
                    "parallelism": f"walkers sharded over {world} GPU(s), no collective",
@@ -470,12 +534,10 @@ def run_cuda(args):
         "accept_fraction": alpha, "gpu_launches": launches, "create_s": create_s,
         "clocks": clk.summary(), "roofline": roofline, "rooflines": extra_rooflines, "kernels": kernels,
     }
-    if rank == 0:
-        try:
-            line["fp64_dgemm_probe_tflops"] = fp64_probe()
-        except Exception as e:  # probe only
-            line["fp64_dgemm_probe_tflops"] = None
-            line["fp64_probe_error"] = str(e)[:80]
+    line["fp64_dgemm_probe_tflops"] = probe
+    line["fp64_dmma_issue_ceiling_tflops"] = FP64_DMMA_CEILING_TFLOPS
+    if probe_err:
+        line["fp64_probe_error"] = probe_err
 
     # end to end through the host-buffer call: H2D positions, rebuild, sweep, D2H positions
     if not args.no_e2e:
@@ -512,13 +574,30 @@ def run_cuda(args):
             avg = kms / cnt
             byts = a1 * W * 16 * wl.n * wl.n
             ent = {"kernel": "rank1", "bound": "hbm", "achieved": byts / (avg * 1e-3) / 1e9, "peak": pk["hbm_gbs"],
-                   "unit": "GB/s", "traffic": traffic.get("rank1"), "avg_us": 1e3 * avg, "accept_fraction": a1,
+                   "unit": "GB/s", "avg_us": 1e3 * avg, "accept_fraction": a1,
                    "probe": "delay_rank 1 crowd, 16 step moves"}
             ent["frac"] = ent["achieved"] / pk["hbm_gbs"]
-            line["rooflines"]["rank1"] = ent
+            line["rooflines"]["rank1"] = with_traffic(ent, "rank1")
         c1.close()
         del c1
         torch.cuda.empty_cache()
+
+    if rank == 0 and world == 1 and args.cfg == 5 and not args.no_sweep_points:
+        # The metric is "electron moves/sec per B200 VS CROWD SIZE" (BASELINE.json; the analogue of the paper's Fig. 5,
+        # P:184 / P:190): a compact sweep inside the parsed line -- crowd sizes at the configured rank, ranks at the
+        # largest crowd; fresh crowd each, 1 warm-up + 2 timed sweeps, acceptance alongside.
+        pts = [(w2, kd) for w2 in (64, 256, 1024) if w2 != W] + [(W, k2) for k2 in (1, 16, 64) if k2 != kd]
+        sweep_pts = [{"walkers": W, "delay_rank": kd, "value": value, "accept_fraction": alpha,
+                      "ms_per_sweep": ms / max(args.steps, 1)}]
+        for W2, k2 in pts:
+            c2, _ = make_crowd(wl, W2, k2, 0, coefs_dev, dev)
+            ms2, prop2, acc2, _ = time_sweeps(c2, 2, 1, torch.cuda.synchronize)
+            sweep_pts.append({"walkers": W2, "delay_rank": k2, "value": prop2 / (ms2 * 1e-3),
+                              "accept_fraction": acc2 / prop2, "ms_per_sweep": ms2 / 2})
+            c2.close()
+            del c2
+            torch.cuda.empty_cache()
+        line["crowd_sweep"] = sorted(sweep_pts, key=lambda r: (r["delay_rank"], r["walkers"]))
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = len(os.sched_getaffinity(0))
@@ -559,8 +638,48 @@ def run_cuda(args):
     return 0
 
 
+def run_plan_only(args):
+    """No GPU work: every rank derives its walker range exactly as run_cuda does and the ranks agree on the plan over
+    gloo; rank 0 prints it.  Lets `--gpus N` (launch, rendezvous, sharding) be tested on a CPU box."""
+    import torch
+    from paper_2209_14487_b200 import dist as qd
+    rank, local_rank, world = qd.env_world()
+    d = qd.init("gloo")
+    id0, cnt = qd.walker_slice(rank, world, args.walkers)
+    mine = torch.tensor([rank, os.getpid(), id0, cnt], dtype=torch.int64)
+    rows = [mine]
+    if world > 1:
+        rows = [torch.zeros(4, dtype=torch.int64) for _ in range(world)]
+        d.all_gather(rows, mine)
+    if rank == 0:
+        print(json.dumps({"plan_only": True, "n_gpus": world, "scaling": "weak",
+                          "ranks": [{"rank": int(r[0]), "pid": int(r[1]), "walker_id0": int(r[2]),
+                                     "walkers": int(r[3])} for r in rows]}), flush=True)
+    if world > 1:
+        d.barrier()
+        d.destroy_process_group()
+    return 0
+
+
+def relaunch_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: start the N ranks here (one process per GPU, rendezvous on
+    127.0.0.1, a free port), exactly the command the driver uses for N > 1."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve())] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return relaunch_ranks(args)
+    if args.plan_only:
+        return run_plan_only(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

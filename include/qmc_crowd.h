@@ -208,8 +208,12 @@ int qmc_crowd_set_option(qmc_crowd_t* crowd, int option, int value);
 #define QMC_OPT_PROFILE 1
 /* option 2 (QMC_OPT_SUBCROWDS): number of sub-crowds (1..4; 0 = automatic, the default: 2 for crowds of one to four
  * waves of window CTAs, else 1) qmc_sweep advances on separate internal
- * streams when delay_rank > 1 (crowds on independent streams overlap); walkers are independent, so
- * results do not depend on it.  The sub-crowds are forked from and joined back into desc.stream every sweep.    */
+ * streams when delay_rank > 1 (crowds on independent streams overlap); walkers are independent and the
+ * threads-per-walker class of the window kernel is chosen from the size of the WHOLE crowd, so results do not depend
+ * on it bit for bit.  (Separate crowds of different sizes may run different classes -- 512 / 256 / 128 threads per
+ * walker for W <= 148 / <= 296 / more -- whose block sums differ at the rounding level: positions and decisions still
+ * agree through the fp32-quantised displacement (D:A7), inverses to ~1e-13.)  The sub-crowds are forked from and joined
+ * back into desc.stream every sweep.                                                                              */
 #define QMC_OPT_SUBCROWDS 2
 /* option 3 (QMC_OPT_RECOMPUTE_EVERY): qmc_sweep / qmc_sweep_host call qmc_recompute_inverse after every `value`-th
  * sweep (counted on the crowd's sweep index, so the schedule does not depend on how sweeps are batched into calls);
@@ -225,11 +229,10 @@ enum {
   QMC_K_RANK1 = 4,       /* Sherman-Morrison rank-1 update (step a4)                             */
   QMC_K_FLUSH = 5,       /* delayed rank-k flush, FP64 DMMA (step a5)                            */
   QMC_K_RATIO_ACCEPT = 6,/* qmc_sweep, delay_rank 1, large n: ratio_grad + accept of electron k  */
-  QMC_K_FUSED_MOVE = 7,  /* (no longer launched; kept so that class numbers stay stable)         */
-  QMC_K_WINDOW = 8,      /* qmc_sweep: all moves of one delay window (or, delay_rank 1 and small n, of a sweep), CTA per walker */
-  QMC_K_KINETIC = 9,     /* qmc_kinetic_energy                                                   */
-  QMC_K_BRANCH = 10,     /* qmc_crowd_branch, qmc_crowd_export / import_walkers (state copies)   */
-  QMC_N_KERNEL_CLASSES = 11
+  QMC_K_WINDOW = 7,      /* qmc_sweep: all moves of one delay window (or, delay_rank 1 and small n, of a sweep), CTA per walker */
+  QMC_K_KINETIC = 8,     /* qmc_kinetic_energy                                                   */
+  QMC_K_BRANCH = 9,      /* qmc_crowd_branch, qmc_crowd_export / import_walkers (state copies)   */
+  QMC_N_KERNEL_CLASSES = 10
 };
 /* Device time (ms, CUDA events on desc.stream) and launch count per kernel class accumulated in
  * profile mode since the previous call; resets the accumulators.  Synchronous.  ms and count

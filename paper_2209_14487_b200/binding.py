@@ -19,7 +19,7 @@ QMC_OPT_PROFILE = 1
 QMC_OPT_SUBCROWDS = 2
 QMC_OPT_RECOMPUTE_EVERY = 3
 KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush", "ratio_accept",
-                  "fused_move", "window", "kinetic", "branch")
+                  "window", "kinetic", "branch")
 
 EXPORTS = [
     "qmc_crowd_workspace_bytes", "qmc_crowd_create", "qmc_crowd_destroy", "qmc_spo_vgl", "qmc_ratio_grad",
@@ -161,27 +161,49 @@ class Crowd:
         self._h = h
 
     # -- the six calls of the boundary -----------------------------------------------------
+    # Outputs are allocated with the crowd's stream current (so the caching allocator ties the block to the stream the
+    # library writes it on) and the caller's current stream is made to wait for the kernels that fill them: a consumer
+    # on another stream never reads an output early when the crowd was built with its own stream (multi-crowd mode).
+    def _on_stream(self):
+        return self.torch.cuda.stream(self.stream)
+
+    def _publish(self, caller_stream):
+        if caller_stream != self.stream:
+            caller_stream.wait_stream(self.stream)
+
     def qmc_spo_vgl(self, k, rnew=None, want_outputs=False):
         t = self.torch
         phi = dphi = d2phi = None
+        caller = t.cuda.current_stream(self.device)
+        if rnew is not None and caller != self.stream:
+            self.stream.wait_stream(caller)            # rnew was produced on the caller's stream
+        with self._on_stream():
+            if want_outputs:
+                phi = t.empty((self.W, self.M), dtype=self.dtype, device=self.device)
+                dphi = t.empty((self.W, 3, self.M), dtype=self.dtype, device=self.device)
+                d2phi = t.empty((self.W, self.M), dtype=self.dtype, device=self.device)
+            _check(load().qmc_spo_vgl(self._h, k, _ptr(rnew, t.float64), _ptr(phi), _ptr(dphi), _ptr(d2phi)))
         if want_outputs:
-            phi = t.empty((self.W, self.M), dtype=self.dtype, device=self.device)
-            dphi = t.empty((self.W, 3, self.M), dtype=self.dtype, device=self.device)
-            d2phi = t.empty((self.W, self.M), dtype=self.dtype, device=self.device)
-        _check(load().qmc_spo_vgl(self._h, k, _ptr(rnew, t.float64), _ptr(phi), _ptr(dphi), _ptr(d2phi)))
+            self._publish(caller)
         return (phi, dphi, d2phi) if want_outputs else None
 
     def qmc_ratio_grad(self, k):
         t = self.torch
-        ratio = t.empty(self.W, dtype=t.float64, device=self.device)
-        grad = t.empty((self.W, 3), dtype=t.float64, device=self.device)
-        _check(load().qmc_ratio_grad(self._h, k, ratio.data_ptr(), grad.data_ptr()))
+        caller = t.cuda.current_stream(self.device)
+        with self._on_stream():
+            ratio = t.empty(self.W, dtype=t.float64, device=self.device)
+            grad = t.empty((self.W, 3), dtype=t.float64, device=self.device)
+            _check(load().qmc_ratio_grad(self._h, k, ratio.data_ptr(), grad.data_ptr()))
+        self._publish(caller)
         return ratio, grad
 
     def qmc_accept_reject(self, k):
         t = self.torch
-        acc = t.empty(self.W, dtype=t.uint8, device=self.device)
-        _check(load().qmc_accept_reject(self._h, k, acc.data_ptr()))
+        caller = t.cuda.current_stream(self.device)
+        with self._on_stream():
+            acc = t.empty(self.W, dtype=t.uint8, device=self.device)
+            _check(load().qmc_accept_reject(self._h, k, acc.data_ptr()))
+        self._publish(caller)
         return acc
 
     def qmc_flush_delayed(self):
@@ -235,10 +257,12 @@ class Crowd:
     def qmc_kinetic_energy(self, per_electron=False):
         """Kinetic energy of every walker, device fp64 [W] (and the per-electron terms [W][N] if asked)."""
         t = self.torch
-        ekin = t.empty((self.W,), dtype=t.float64, device=self.device)
-        e = t.empty((self.W, self.N), dtype=t.float64, device=self.device) if per_electron else None
-        with t.cuda.stream(self.stream):
+        caller = t.cuda.current_stream(self.device)
+        with self._on_stream():
+            ekin = t.empty((self.W,), dtype=t.float64, device=self.device)
+            e = t.empty((self.W, self.N), dtype=t.float64, device=self.device) if per_electron else None
             _check(load().qmc_kinetic_energy(self._h, ekin.data_ptr(), e.data_ptr() if per_electron else None))
+        self._publish(caller)
         return (ekin, e) if per_electron else ekin
 
     # -- state access ------------------------------------------------------------------------

@@ -182,6 +182,8 @@ int check_desc(const qmc_crowd_desc* ds)
   if (ds->n_elec < 2 || (ds->n_elec & 1)) return fail(QMC_ERR_INVALID_ARG, "n_elec must be even and >= 2");
   if (ds->n_orb != ds->n_elec / 2) return fail(QMC_ERR_INVALID_ARG, "n_orb must equal n_elec/2");
   if (ds->n_walkers < 1) return fail(QMC_ERR_INVALID_ARG, "n_walkers must be >= 1");
+  // several kernels put W (or 2 W) in gridDim.y, which CUDA limits to 65535
+  if (ds->n_walkers > 32767) return fail(QMC_ERR_INVALID_ARG, "n_walkers must be <= 32767 per crowd (split the population into crowds)");
   if (ds->coef_dtype != 0 && ds->coef_dtype != 1) return fail(QMC_ERR_INVALID_ARG, "coef_dtype must be 0 or 1");
   if (ds->delay_rank < 1 || ds->delay_rank > 64) return fail(QMC_ERR_INVALID_ARG, "delay_rank must be in [1,64]");
   const int vw = ds->coef_dtype ? 2 : 4;
@@ -211,7 +213,6 @@ int launch_build_t(qmc_crowd* c)
   const size_t blocks = (size_t)d.W * d.N;
   if (blocks > 0x7fffffffull) return fail(QMC_ERR_INVALID_ARG, "crowd too large for one build launch");
   const size_t smem = (size_t)5 * d.ns * sizeof(T);
-  if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(spline_build_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int* order = nullptr;
 #ifndef QMC_BUILD_UNSORTED
   if (d.cell_bins && blocks >= 256) {
@@ -247,19 +248,12 @@ int rebuild(qmc_crowd* c)
   c->launches += 3;
   int st = c->is_f64 ? launch_build_t<double>(c) : launch_build_t<float>(c);
   if (st) return st;
-  const size_t bsmem = invert_blocked_smem(d.ns), b2smem = invert_blocked2_smem(d.ns);
-#ifndef QMC_INVERT_V1
+  const size_t b2smem = invert_blocked2_smem(d.ns);
   if (b2smem <= 227 * 1024 && d.ns <= 2 * INVB2_NT) {
-    if (b2smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_blocked2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b2smem));
     invert_blocked2_kernel<<<(unsigned)(d.W * 2), INVB2_NT, b2smem, c->stream>>>(d);
-  } else
-#endif
-  if (bsmem <= 227 * 1024 && d.ns <= INVB_NT) {
-    if (bsmem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_blocked_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsmem));
-    invert_blocked_kernel<<<(unsigned)(d.W * 2), INVB_NT, bsmem, c->stream>>>(d);
   } else {
+    // matrices too large for the shared-memory panel: the unblocked Gauss-Jordan (same pivots, 2 n sweeps of the matrix)
     const size_t smem = (size_t)(2 * d.ns + 2 * (INV_NT / 32)) * 8 + (size_t)d.ns * 4 + 64;
-    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     invert_kernel<<<(unsigned)(d.W * 2), INV_NT, smem, c->stream>>>(d);
   }
   LAUNCH_CHECK(c);
@@ -423,6 +417,7 @@ int launch_ratio_accept_t(qmc_crowd* c, int k)
 size_t window_smem(const CrowdDev& d, size_t elem, int nt = MOVE_NT) { return (size_t)win_layout(d.N, d.ns, d.kdp, (int)elem, nt).total * 8; }
 
 // Threads per walker of the window kernel: a crowd that leaves SMs idle gets wider CTAs (shorter move chain).
+// W = the whole crowd's size (sub-crowds of qmc_sweep keep their crowd's class, so QMC_OPT_SUBCROWDS is bit-invariant).
 int window_threads(int wn) { return wn <= 148 ? 512 : (wn <= 296 ? 256 : 128); }
 
 template <typename T>
@@ -431,7 +426,7 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   ProfScope ps(c, QMC_K_WINDOW);
   CrowdDev d = c->dev;
   d.w0 = w0;
-  switch (window_threads(wn)) {
+  switch (window_threads(d.W)) {   // the class of the WHOLE crowd: a split into sub-crowds never changes a reduction tree
     case 512: window_kernel<T, 512><<<wn, 512, window_smem(d, sizeof(T), 512), st>>>(d, k0, cnt); break;
     case 256: window_kernel<T, 256><<<wn, 256, window_smem(d, sizeof(T), 256), st>>>(d, k0, cnt); break;
     default: window_kernel<T, 128><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt); break;
@@ -440,17 +435,46 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   return QMC_OK;
 }
 
-template <typename T>
-cudaError_t window_smem_attr(const CrowdDev& d)
+// Dynamic shared memory above 48 KB is an opt-in attribute of each kernel, and it is process-wide: it is raised ONCE
+// per device to what the device allows (minus the kernel's static shared memory), never to one crowd's need, so that
+// crowds of different shapes in one process cannot lower it under each other's launches.
+cudaError_t raise_smem_limit(const void* fn, int optin)
 {
-  cudaError_t e = cudaSuccess;
-  const int s128 = (int)window_smem(d, sizeof(T), 128), s256 = (int)window_smem(d, sizeof(T), 256),
-            s512 = (int)window_smem(d, sizeof(T), 512);
-  if (s128 > 48 * 1024) e = cudaFuncSetAttribute(window_kernel<T, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128);
-  if (e == cudaSuccess && s256 > 48 * 1024) e = cudaFuncSetAttribute(window_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, s256);
-  if (e == cudaSuccess && s512 > 48 * 1024) e = cudaFuncSetAttribute(window_kernel<T, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, s512);
-  if (e == cudaSuccess && s128 > 48 * 1024) e = cudaFuncSetAttribute(sweep1_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128);
-  return e;
+  cudaFuncAttributes a;
+  cudaError_t e = cudaFuncGetAttributes(&a, fn);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)a.sharedSizeBytes);
+}
+
+template <typename T>
+cudaError_t raise_smem_limits_t(int optin)
+{
+  const void* fns[] = {(const void*)row_propose_kernel<T>, (const void*)ratio_grad_kernel<T>, (const void*)accept_kernel<T>,
+                       (const void*)ratio_accept_kernel<T>, (const void*)window_kernel<T, 128>,
+                       (const void*)window_kernel<T, 256>, (const void*)window_kernel<T, 512>,
+                       (const void*)sweep1_kernel<T>, (const void*)spline_build_kernel<T>, (const void*)kinetic_kernel<T>};
+  for (const void* f : fns) {
+    cudaError_t e = raise_smem_limit(f, optin);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t raise_smem_limits()
+{
+  static bool done[64] = {};
+  int dev = 0, optin = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+  e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return e;
+  if ((e = raise_smem_limits_t<float>(optin)) != cudaSuccess) return e;
+  if ((e = raise_smem_limits_t<double>(optin)) != cudaSuccess) return e;
+  if ((e = raise_smem_limit((const void*)invert_blocked2_kernel, optin)) != cudaSuccess) return e;
+  if ((e = raise_smem_limit((const void*)invert_kernel, optin)) != cudaSuccess) return e;
+  if (dev >= 0 && dev < 64) done[dev] = true;
+  return cudaSuccess;
 }
 
 // One full sweep with the D:C6 flush schedule; no host synchronisation (capturable).
@@ -641,16 +665,7 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
     const int sm = (int)move_smem(d), wsm = (int)window_smem(d, c->elem, 512);
     if (wsm > 227 * 1024 || sm > 227 * 1024)
       return bail(fail(QMC_ERR_INVALID_ARG, "n_elec / delay_rank too large: the per-walker state (%d bytes) exceeds shared memory", wsm));
-    const void* fns[] = {(const void*)row_propose_kernel<float>, (const void*)row_propose_kernel<double>,
-                         (const void*)ratio_grad_kernel<float>, (const void*)ratio_grad_kernel<double>,
-                         (const void*)accept_kernel<float>, (const void*)accept_kernel<double>,
-                         (const void*)ratio_accept_kernel<float>, (const void*)ratio_accept_kernel<double>};
-    for (const void* f : fns) {
-      if (sm <= 48 * 1024) break;
-      e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-      if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
-    }
-    e = c->is_f64 ? window_smem_attr<double>(d) : window_smem_attr<float>(d);
+    e = raise_smem_limits();
     if (e != cudaSuccess) return bail(fail(QMC_ERR_CUDA, "smem attribute: %s", cudaGetErrorString(e)));
   }
   st = rebuild(c);
@@ -934,10 +949,8 @@ int qmc_kinetic_energy(qmc_crowd_t* c, double* ekin_dev, double* e_elec_dev)
   {
     ProfScope ps(c, QMC_K_KINETIC);
     if (c->is_f64) {
-      if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(kinetic_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       kinetic_kernel<double><<<grid, EKIN_NT, smem, c->stream>>>(d, d.e_elec);
     } else {
-      if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(kinetic_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       kinetic_kernel<float><<<grid, EKIN_NT, smem, c->stream>>>(d, d.e_elec);
     }
     LAUNCH_CHECK(c);

@@ -37,3 +37,57 @@ def relerr(x, y):
 
 def npy(t):
     return t.detach().cpu().numpy()
+
+
+def straddle_flags(log, tau, g_tol=1e-10):
+    """Which logged moves have a displacement whose fp32 rounding (reading A7) is decided by less than a relative
+    error g_tol of G_k(R)?  log: oracle move records [...]; returns a bool array of the same shape.
+
+    Delta_c = fl32(x_c), x_c = tau G_c + sqrt(tau) chi_c.  Two correct fp64 implementations agree on G to g_tol
+    (relative to max_c |G_c|; BASELINE.json: 1e-10) and on chi to a few ulp of libm, so their x_c differ by at most
+    e = g_tol tau max|G| + 8 eps |x|; the roundings can differ only if x_c lies within e of a rounding boundary,
+    i.e. if the oracle's margin (in fp32 ulps of Delta_c, minimum over components) is below e / ulp32(Delta_c)."""
+    delta, g, margin = log["delta"], log["g_old"], log["disp_margin"]
+    e = g_tol * tau * np.abs(g).max(axis=-1) + 8 * 2.0 ** -53 * np.abs(delta).max(axis=-1)
+    ulp = np.spacing(np.abs(delta).astype(np.float32)).astype(np.float64)
+    return margin < (e[..., None] / ulp).max(axis=-1)
+
+
+class FreeRunningCheck:
+    """P-free with classification: a free-running trajectory of the CUDA path against the
+    oracle's, sweep by sweep, for crowds too long for "no rounding tie anywhere" to be a property of the inputs.
+
+    Within a sweep every electron is proposed once, so the positions after the sweep show move by move where the two
+    sides differ.  For every walker, all moves before its first difference agree bit for bit; that first difference
+    must be a move whose fp32 displacement rounding the oracle itself reports as decided by less than the parity
+    tolerance on G (straddle_flags) -- anything else is a bug and fails.  A walker that has met such a straddle has
+    departed from the oracle's trajectory by one fp32 ulp of one displacement (~1e-8) and is from then on compared for
+    closeness only (positions 1e-6, inverses 1e-5, same accept / reject decisions)."""
+
+    def __init__(self, W, tau, g_tol=1e-10):
+        self.tau, self.g_tol = tau, g_tol
+        self.departed = np.zeros(W, dtype=bool)
+        self.exact_moves = 0
+
+    def sweep(self, Rg_prev, Rg, Ro_prev, Ro, log):
+        """Rg_prev / Rg: CUDA positions before / after the sweep, Ro_prev / Ro: the oracle's; log: [W][N] records."""
+        flags = straddle_flags(log, self.tau, self.g_tol)
+        W, N = log.shape
+        for w in range(W):
+            diff = np.any(Rg[w] != Ro[w], axis=-1)
+            if not self.departed[w]:
+                if diff.any():
+                    k = int(np.argmax(diff))
+                    assert flags[w, k], (f"walker {w}, electron {k}: positions differ although the oracle's rounding "
+                                         f"margin ({log[w, k]['disp_margin']:.3e} fp32 ulps) rules out a straddle")
+                    self.departed[w] = True
+                    self.exact_moves += k
+                else:
+                    self.exact_moves += N
+            assert np.abs(Rg[w] - Ro[w]).max() < 1e-6, f"walker {w} left the oracle's trajectory"
+            moved_g, moved_o = np.any(Rg[w] != Rg_prev[w], axis=-1), np.any(Ro[w] != Ro_prev[w], axis=-1)
+            tie = np.abs(log[w]["u"] - log[w]["p"]) <= 1e-5 * np.abs(log[w]["p"])
+            assert np.array_equal(moved_g[~tie], moved_o[~tie]), f"walker {w}: accept / reject decisions differ"
+
+    def inverse_tol(self, w):
+        return 1e-5 if self.departed[w] else 1e-10
