@@ -8,10 +8,10 @@
 // Work split (one CTA evaluates one position; the same device function serves qmc_spo_vgl, the
 // Slater build at create and the walker-persistent window kernel of qmc_sweep):
 //   an item = (16-byte orbital slice, x-plane a): 16 independent 16-byte loads (4 y x 4 z rows),
-//   contracted z -> y in registers, scaled by the x weights of plane a.  The four planes of a slice
-//   sit in four adjacent lanes and are summed by two xor-shuffles, so a warp request is four runs
-//   of 128 contiguous bytes (8 slices x 16 B per plane) and every thread keeps 16 loads in flight
-//   with ~64 data registers -- the 64-loads-per-thread form needed 153 registers (3 CTAs/SM).
+//   contracted z -> y in registers, scaled by the x weights of plane a.  A warp takes 8 slices x 4 planes
+//   (lane = 8 a + slice): a warp request is four runs of 128 contiguous bytes, one per quarter-warp, the
+//   four planes of a slice are summed by two xor-shuffles (8, 16), and every thread keeps 16 loads in
+//   flight with ~64 data registers -- the 64-loads-per-thread form needed 153 registers (3 CTAs/SM).
 #pragma once
 #include "common.cuh"
 
@@ -124,6 +124,58 @@ __device__ __forceinline__ void spline_plane_sum(const SplineW<T>& s, int a, con
   }
 }
 
+// The same contraction for an fp32 table with packed arithmetic (sm_100 FFMA2 / FMUL2 / FADD2: two IEEE operations
+// per instruction on a register pair): element for element the same products and sums in the same order as the generic
+// version, i.e. bit-identical results with half the floating-point instructions (they were a quarter of the window
+// kernel's instruction stream, which is what bounds it: ncu r2).
+__device__ __forceinline__ void spline_plane_sum(const SplineW<float>& s, int a, const float (&p)[4][4][4], float (&out)[5][4])
+{
+  float2 u00[2], u10[2], u20[2], u01[2], u02[2];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) u00[h] = u10[h] = u20[h] = u01[h] = u02[h] = make_float2(0.f, 0.f);
+  float2 wz[4], dwz[4], d2wz[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    wz[c] = make_float2(s.w[2][c], s.w[2][c]);
+    dwz[c] = make_float2(s.dw[2][c], s.dw[2][c]);
+    d2wz[c] = make_float2(s.d2w[2][c], s.d2w[2][c]);
+  }
+#pragma unroll
+  for (int b = 0; b < 4; ++b) {
+    const float2 wy = make_float2(s.w[1][b], s.w[1][b]), dwy = make_float2(s.dw[1][b], s.dw[1][b]),
+                 d2wy = make_float2(s.d2w[1][b], s.d2w[1][b]);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const float2 p0 = make_float2(p[b][0][2 * h], p[b][0][2 * h + 1]);
+      float2 v0 = __fmul2_rn(wz[0], p0), v1 = __fmul2_rn(dwz[0], p0), v2 = __fmul2_rn(d2wz[0], p0);
+#pragma unroll
+      for (int c = 1; c < 4; ++c) {
+        const float2 pc = make_float2(p[b][c][2 * h], p[b][c][2 * h + 1]);
+        v0 = __ffma2_rn(wz[c], pc, v0);
+        v1 = __ffma2_rn(dwz[c], pc, v1);
+        v2 = __ffma2_rn(d2wz[c], pc, v2);
+      }
+      u00[h] = __ffma2_rn(wy, v0, u00[h]);
+      u10[h] = __ffma2_rn(dwy, v0, u10[h]);
+      u20[h] = __ffma2_rn(d2wy, v0, u20[h]);
+      u01[h] = __ffma2_rn(wy, v1, u01[h]);
+      u02[h] = __ffma2_rn(wy, v2, u02[h]);
+    }
+  }
+  const float2 wa = make_float2(s.w[0][a], s.w[0][a]), dwa = make_float2(s.dw[0][a], s.dw[0][a]),
+               d2wa = make_float2(s.d2w[0][a], s.d2w[0][a]);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const float2 o0 = __fmul2_rn(wa, u00[h]), o1 = __fmul2_rn(dwa, u00[h]), o2 = __fmul2_rn(wa, u10[h]),
+                 o3 = __fmul2_rn(wa, u01[h]), o4 = __ffma2_rn(d2wa, u00[h], __fmul2_rn(wa, __fadd2_rn(u20[h], u02[h])));
+    out[0][2 * h] = o0.x; out[0][2 * h + 1] = o0.y;
+    out[1][2 * h] = o1.x; out[1][2 * h + 1] = o1.y;
+    out[2][2 * h] = o2.x; out[2][2 * h + 1] = o2.y;
+    out[3][2 * h] = o3.x; out[3][2 * h + 1] = o3.y;
+    out[4][2 * h] = o4.x; out[4][2 * h + 1] = o4.y;
+  }
+}
+
 __device__ __forceinline__ float shfl_xor_t(float v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 __device__ __forceinline__ double shfl_xor_t(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 
@@ -135,12 +187,17 @@ __device__ __forceinline__ double shfl_xor_t(double v, int m) { return __shfl_xo
 struct NoSideWork { __device__ __forceinline__ void operator()(int) const {} };
 // r == nullptr: the caller has already filled `s` for this position (spline_axis per axis).
 // KEEP: loads without the L2 evict-first hint (callers that arrange for L2 re-use).
-template <typename T, int NT, typename Side = NoSideWork, bool KEEP = false>
+// PRESYNCED: the caller has already synchronised after filling `s` (and may have done work of its own in between).
+template <typename T, int NT, typename Side = NoSideWork, bool KEEP = false, bool PRESYNCED = false>
 __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, SplineW<T>& s, T* vgl, Side side = Side())
 {
   constexpr int VW = Vec16<T>::W;
-  const int tid = threadIdx.x, a = tid & 3, g = tid >> 2;
-  __syncthreads();  // previous users of `s` are done / the caller's weights are visible
+  // lane = 8 a + slice: the eight lanes of a quarter-warp read eight adjacent 16-byte slices of ONE row (one 128-byte
+  // line = one L1 wavefront per quarter-warp of a 128-bit load; with the four planes in adjacent lanes a quarter-warp
+  // touched four lines and the gather cost four times the wavefronts -- the L1 data pipe was the busiest unit of the
+  // window kernel, ncu r2).  The planes of a slice sit 8 and 16 lanes apart.
+  const int tid = threadIdx.x, lane = tid & 31, a = lane >> 3, g = (tid >> 5) * 8 + (lane & 7);
+  if (!PRESYNCED) __syncthreads();  // previous users of `s` are done / the caller's weights are visible
   if (r) {
     if (tid < 3) spline_axis<T>(d, tid, r[tid], s);
     __syncthreads();
@@ -155,7 +212,7 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
       T p[4][4][VW];
       spline_plane_load<T, KEEP>(tab, s, a, chunk, p);
       if (c0 == 0 && tid >= 32) side(tid);
-      spline_plane_sum<T>(s, a, p, out);
+      spline_plane_sum(s, a, p, out);
     } else {
       if (c0 == 0 && tid >= 32) side(tid);
 #pragma unroll
@@ -163,8 +220,8 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
 #pragma unroll
         for (int e = 0; e < VW; ++e) out[q][e] = (T)0;
     }
-    // Sum over the four planes (lanes a = 0..3) with the owner of each quantity as the only receiver: lane a ends
-    // up with quantity a, lane 0 also with the laplacian.  Same pairwise tree per value as two full xor-shuffles,
+    // Sum over the four planes (lanes 8 a + slice) with the owner of each quantity as the only receiver: plane a's lane
+    // ends up with quantity a, plane 0's also with the laplacian.  Same pairwise tree per value as two full xor-shuffles,
     // (p_a + p_{a^1}) + (p_{a^2} + p_{a^3}), with 5 instead of 10 shuffles per value.
     const bool odd = a & 1, up = a & 2;
     T r0[VW], r1[VW], r2[VW];  // after step 1: even lanes hold q0, q2, q4; odd lanes hold q1, q3 (r2 unused)
@@ -172,17 +229,17 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
     for (int e = 0; e < VW; ++e) {
       const T s0 = odd ? out[0][e] : out[1][e], s1 = odd ? out[2][e] : out[3][e], s2 = odd ? out[4][e] : (T)0;
       const T k0 = odd ? out[1][e] : out[0][e], k1 = odd ? out[3][e] : out[2][e], k2 = out[4][e];
-      r0[e] = k0 + shfl_xor_t(s0, 1);
-      r1[e] = k1 + shfl_xor_t(s1, 1);
-      r2[e] = k2 + shfl_xor_t(s2, 1);
+      r0[e] = k0 + shfl_xor_t(s0, 8);
+      r1[e] = k1 + shfl_xor_t(s1, 8);
+      r2[e] = k2 + shfl_xor_t(s2, 8);
     }
     T f0[VW], f1[VW];  // after step 2: lane 0: q0, q4; lane 1: q1; lane 2: q2; lane 3: q3
 #pragma unroll
     for (int e = 0; e < VW; ++e) {
       const T s0 = up ? r0[e] : r1[e], s1 = up ? r2[e] : (T)0;
       const T k0 = up ? r1[e] : r0[e], k1 = r2[e];
-      f0[e] = k0 + shfl_xor_t(s0, 2);
-      f1[e] = k1 + shfl_xor_t(s1, 2);
+      f0[e] = k0 + shfl_xor_t(s0, 16);
+      f1[e] = k1 + shfl_xor_t(s1, 16);
     }
 #pragma unroll
     for (int e = 0; e < VW; ++e)
@@ -192,6 +249,25 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
       st16(o + (size_t)a * d.ns, f0);
       if (a == 0) st16(o + (size_t)4 * d.ns, f1);
     }
+  }
+}
+
+// L2 prefetch of the 64 stencil rows of the position whose weights are in `s` (a row = the orbitals of one grid point,
+// contiguous): every thread asks for its share of the rows' 128-byte lines.  prefetch.global.L2 moves DRAM -> L2
+// without occupying a register or a load slot: the gather that follows finds its lines in, or on their way to, L2.
+// (cp.async.bulk.prefetch.L2, one instruction per row, takes its address from a uniform register: ptxas serialises
+// it lane by lane -- 2.5 % of the window kernel's instructions when tried.)
+template <typename T, int NT>
+__device__ __forceinline__ void spline_prefetch_l2(const CrowdDev& d, const SplineW<T>& s)
+{
+  constexpr int VW = Vec16<T>::W;
+  const unsigned vecs = d.tab_vecs < (unsigned)d.ns / VW ? d.tab_vecs : (unsigned)d.ns / VW;
+  const unsigned lines = (vecs + 7) / 8;   // 128-byte lines per row
+  const char* tab = static_cast<const char*>(d.coefs);
+  for (unsigned e = threadIdx.x; e < 64 * lines; e += NT) {
+    const unsigned row = e / lines, ln = e - row * lines;
+    const size_t vec = (size_t)(s.off[0][row >> 4] + s.off[1][(row >> 2) & 3] + s.off[2][row & 3]) + 8 * ln;
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(tab + vec * 16));
   }
 }
 

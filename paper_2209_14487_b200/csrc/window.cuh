@@ -29,7 +29,7 @@ namespace qmc {
 
 // Shared-memory layout of the window kernel, offsets in doubles.
 struct WinLayout {
-  int R, b, bn, red, mv, gauss, rows, cbuf, vgl, total;
+  int R, b, bn, red, mv, gauss, pairk, rows, cbuf, vgl, total;
 };
 __host__ __device__ inline WinLayout win_layout(int N, int ns, int kdp, int elem, int nt = MOVE_NT)
 {
@@ -41,9 +41,14 @@ __host__ __device__ inline WinLayout win_layout(int N, int ns, int kdp, int elem
   L.red = o; o += (8 * (nt / 32) < 32 ? 32 : 8 * (nt / 32));
   L.mv = o; o += MOVE_MV;
   L.gauss = o; o += 8;       // Box-Muller pieces of the next move
+  L.pairk = o; o += 8;       // the pair term (k+1, k) against r_k and against r'_k (window kernel)
   L.rows = o; o += kdp / 2;  // int[kdp]: electron (within the spin block) of accepted move l
   o = (o + 1) & ~1;
+#ifdef QMC_WIN_CBUF1
+  L.cbuf = o; o += ((3 * ns * elem + 15) / 16) * 2;      // gradient cache of the coming move: T[3][ns]
+#else
   L.cbuf = o; o += 2 * ((3 * ns * elem + 15) / 16) * 2;  // gradient cache of this / the next move: 2 x T[3][ns]
+#endif
   L.vgl = o; o += (5 * ns * elem + 7) / 8;               // orbitals at r': T[5][ns]
   L.total = o;
   return L;
@@ -69,6 +74,131 @@ template <int NT = MOVE_NT>
 __device__ __forceinline__ void cp_async_cta(void* smem, const void* gmem, int nbytes)
 {
   for (int o = threadIdx.x * 16; o < nbytes; o += NT * 16)
+    cp_async16(static_cast<char*>(smem) + o, static_cast<const char*>(gmem) + o);
+}
+
+// ---- the Jastrow sums of a move, taken off the walker's critical path ---------------------------------------------
+// A move needs two pair sums (D:C3): at the current position r_k for G_k(R) (proposal) and at r' for the ratio.  Both
+// are ~70 dependent fp64 instructions per pair, six pairs per thread: next to the row dots they were 2 x 3000 cycles
+// of every move's chain.  Neither depends on what the move itself decides, except through one pair term:
+//   - the sum at r' needs only r' and R: it is evaluated right after the proposal, while the stencil rows of r' are
+//     on their way from DRAM to L2 (spline_prefetch_l2);
+//   - the sum at r_{k+1} for the NEXT move is evaluated at the same time over all electrons but k (whose position the
+//     pending decision may change); the missing term is evaluated for both outcomes (against r_k and against r'_k)
+//     and the one that applies is added after the decision.
+struct J2Part {
+  double us, g[3];
+};
+// One pair term, branch-free (the same products and the same order of operations as j2_pair; `on` = false contributes
+// exact zeros): straight-line code lets the scheduler interleave several pairs -- a pair is a chain of ~45 dependent
+// fp64 instructions, and a thread that walks its pairs one after the other issues one instruction per ~12 cycles.
+__device__ __forceinline__ void j2_pair_bf(const CrowdDev& d, const double (&rk)[3], const double* ri, bool on, J2Part& s)
+{
+  double dd[3], r2 = 0.0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    double x = rk[c] - ri[c];
+    x -= d.box[c] * rint(x * d.inv_box[c]);
+    dd[c] = x;
+    r2 = fma(x, x, r2);
+  }
+  on = on && r2 > 1e-280;
+  const double inv_r = rsqrt_pos(on ? r2 : 1.0);
+  const double r = r2 * inv_r;
+  const double inv_den = rcp_pos(fma(d.j2_b, r, 1.0));
+  const double a = on ? d.j2_a : 0.0;
+  s.us += a * r * inv_den;
+  const double f = a * inv_den * inv_den * inv_r;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) s.g[c] = fma(f, dd[c], s.g[c]);
+}
+
+// Thread-strided partials of two pair sums at once: electron k placed at rn against all electrons but k, and (if
+// `next`) electron k + 1 at its own position rk1 against all electrons but k and k + 1.  Two electrons per trip, so
+// four independent pair chains are in flight per thread.
+template <int NT>
+__device__ __forceinline__ void j2_two_sums(const CrowdDev& d, const double* R, int k, const double (&rn)[3], bool next,
+                                            const double (&rk1)[3], J2Part& at_rn, J2Part& at_next)
+{
+  at_rn.us = at_rn.g[0] = at_rn.g[1] = at_rn.g[2] = 0.0;
+  at_next.us = at_next.g[0] = at_next.g[1] = at_next.g[2] = 0.0;
+  const int N = d.N;
+  for (int i0 = threadIdx.x; i0 < N; i0 += 2 * NT) {
+    const int i1 = i0 + NT;
+    const bool in1 = i1 < N;
+    const double* ra = R + 3 * i0;
+    const double* rb = R + 3 * (in1 ? i1 : i0);
+    j2_pair_bf(d, rn, ra, i0 != k, at_rn);
+    j2_pair_bf(d, rk1, ra, next && i0 != k && i0 != k + 1, at_next);
+    j2_pair_bf(d, rn, rb, in1 && i1 != k, at_rn);
+    j2_pair_bf(d, rk1, rb, next && in1 && i1 != k && i1 != k + 1, at_next);
+  }
+}
+
+// G_k(R) and the proposal from the row dots and a precomputed Jastrow partial (see dev_gold_propose for the formulas;
+// same products, the pair terms summed in a different order).  extra: the pair term (k, k-1) chosen after the previous
+// decision, added by thread 0 (nullptr for the first move of a window).
+template <typename T, int NT>
+__device__ __forceinline__ void win_gold_propose(const CrowdDev& d, int k, const double* b_s, const T* cache, const double* R,
+                                                 const J2Part& jp, const double* extra, MoveScal ms, double* red,
+                                                 const double* gp, SplineW<T>* sw_out)
+{
+  const int ns = d.ns, tid = threadIdx.x;
+  double v[7] = {0.0, 0.0, 0.0, jp.us, jp.g[0], jp.g[1], jp.g[2]};
+  for (int j = tid; j < d.M; j += NT) {
+    const double bj = b_s[j];
+    v[0] = fma(bj, (double)cache[j], v[0]);
+    v[1] = fma(bj, (double)cache[ns + j], v[1]);
+    v[2] = fma(bj, (double)cache[2 * ns + j], v[2]);
+  }
+  if (extra && tid == 0) {
+    v[3] += extra[0]; v[4] += extra[1]; v[5] += extra[2]; v[6] += extra[3];
+  }
+  block_sum_t0<7, NT>(v, red);
+  if (tid < 3) {
+    const int c = tid;
+    const double g_old = c == 0 ? v[0] + v[4] : (c == 1 ? v[1] + v[5] : v[2] + v[6]);
+    const double rkc = R[3 * k + c];
+    const double chi = c == 0 ? gp[0] * gp[1] : (c == 1 ? gp[0] * gp[2] : gp[3] * gp[4]);
+    const double xx = __dadd_rn(__dmul_rn(d.tau, g_old), __dmul_rn(d.sqrt_tau, chi));
+    const double delta = (double)__double2float_rn(xx);
+    const double rn = rkc + delta;
+    ms.g_old[c] = g_old;
+    ms.delta[c] = delta;
+    ms.rn[c] = rn;
+    if (c == 0) *ms.usum_old = v[3];
+    spline_axis<T>(d, c, rn, *sw_out);
+  }
+}
+
+// rho_D, rho_J and G_k(R') from the row dots and the precomputed Jastrow partial at r' (see dev_ratio_grad).
+template <typename T, int NT>
+__device__ __forceinline__ void win_ratio_grad(const CrowdDev& d, const double* b, const T* vgl, const J2Part& jr,
+                                               MoveScal ms, double* red)
+{
+  const int ns = d.ns, tid = threadIdx.x;
+  double v[8] = {0.0, 0.0, 0.0, 0.0, jr.us, jr.g[0], jr.g[1], jr.g[2]};
+  for (int j = tid; j < d.M; j += NT) {
+    const double bj = b[j];
+    v[0] = fma(bj, (double)vgl[j], v[0]);
+    v[1] = fma(bj, (double)vgl[ns + j], v[1]);
+    v[2] = fma(bj, (double)vgl[2 * ns + j], v[2]);
+    v[3] = fma(bj, (double)vgl[3 * ns + j], v[3]);
+  }
+  block_sum_t0<8, NT>(v, red);
+  if (tid == 0) {
+    const double rho_d = v[0];
+    *ms.rho_d = rho_d;
+    *ms.rho_j = exp(v[4] - *ms.usum_old);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) ms.g_new[c] = v[1 + c] / rho_d + v[5 + c];
+  }
+}
+
+// the same by one warp (a warp that would otherwise idle at a barrier)
+__device__ __forceinline__ void cp_async_warp(void* smem, const void* gmem, int nbytes)
+{
+  for (int o = (threadIdx.x & 31) * 16; o < nbytes; o += 32 * 16)
     cp_async16(static_cast<char*>(smem) + o, static_cast<const char*>(gmem) + o);
 }
 
@@ -152,8 +282,11 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
 // Leaves for the flush: V[l] = phi_l, Cp[l] = c_l, rows[l], mwin (and Bcur in the d.C buffer, dead afterwards).
 // NT threads per walker: 128 for full crowds (4 CTAs/SM), 256 / 512 when the crowd leaves SMs idle (a move is then a
 // latency chain and wider CTAs shorten every phase of it: +10 % at W = 256, +35 % at W = 64 on cfg 5).
+#ifndef QMC_WIN_MINCTAS
+#define QMC_WIN_MINCTAS 4
+#endif
 template <typename T, int NT>
-__global__ void __launch_bounds__(NT, 512 / NT) window_kernel(CrowdDev d, int k0, int cnt)
+__global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) window_kernel(CrowdDev d, int k0, int cnt)
 {
   extern __shared__ double sm[];
   __shared__ SplineW<T> sw;
@@ -164,6 +297,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) window_kernel(CrowdDev d, int k0
   double* bn_s = sm + L.bn;  // row of the next move
   double* red = sm + L.red;
   double* gauss = sm + L.gauss;
+  double* pairk = sm + L.pairk;
   int* rows_s = reinterpret_cast<int*>(sm + L.rows);
   const int cstride = ((3 * ns * (int)sizeof(T) + 15) / 16) * 16 / (int)sizeof(T);
   T* cbuf = reinterpret_cast<T*>(sm + L.cbuf);
@@ -189,26 +323,83 @@ __global__ void __launch_bounds__(NT, 512 / NT) window_kernel(CrowdDev d, int k0
     asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
   cp_async_wait_all();
   __syncthreads();
+  J2Part jnext;   // Jastrow partial of the coming move's electron at its current position
+  {
+    const double rk0[3] = {R_s[3 * k0], R_s[3 * k0 + 1], R_s[3 * k0 + 2]};
+    jnext.us = jnext.g[0] = jnext.g[1] = jnext.g[2] = 0.0;
+    j2_partial<NT>(d, R_s, k0, rk0, jnext.us, jnext.g);
+  }
 
-  int m = 0;
+#ifdef QMC_PHASE_CLOCKS
+  long long ph_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, ph_c = clock64();
+#define PH(x) do { if (tid == 0) { const long long c_ = clock64(); ph_t[x] += c_ - ph_c; ph_c = c_; } } while (0)
+#else
+#define PH(x) do {} while (0)
+#endif
+  int m = 0, prev_acc = 0;
   for (int i = 0; i < cnt; ++i) {
     const int k = k0 + i;
+#ifdef QMC_WIN_CBUF1
+    T* ccur = cbuf;
+#else
     T* ccur = cbuf + (i & 1) * cstride;
+#endif
     T* cache_g = cache0 + (size_t)i * 4 * ns;
     const bool more = i + 1 < cnt;
-    if (more) {  // next move's row (valid unless this move is accepted, which rewrites it) and gradient cache
-      cp_async_cta<NT>(bn_s, (m ? Bcur : blk) + (size_t)(i + 1) * ns, row_bytes);
-      cp_async_cta<NT>(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
-    }
-    // ---- G_k(R), proposal, orbitals at r' (the next move's Gaussians ride along), ratio, decision ----
-    dev_gold_propose<T, NT>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss, &sw);
-    spline_cta<T, NT>(d, nullptr, sw, vgl_s, [&](int t) {
-      if (more && t < 37) gauss[t - 32] = gauss_piece(d, w, k + 1, t - 32);
-    });
+    PH(0);
+    // ---- G_k(R) and the proposal: row dots + the Jastrow partial prepared during the previous move ----
+    win_gold_propose<T, NT>(d, k, b_s, ccur, R_s, jnext, i ? pairk + 4 * prev_acc : nullptr, ms, red, gauss, &sw);
+    __syncthreads();   // r' and the spline weights of r' are visible
+    PH(1);
+    // ---- stencil rows of r' towards L2; in their shadow both Jastrow sums ----
+    spline_prefetch_l2<T, NT>(d, sw);
+    J2Part jr;
+    const double rn[3] = {ms.rn[0], ms.rn[1], ms.rn[2]};
+    const int k1 = more ? k + 1 : k;
+    const double rk1[3] = {R_s[3 * k1], R_s[3 * k1 + 1], R_s[3 * k1 + 2]};
+#ifdef QMC_EXP_NOJ2
+    jr.us = jr.g[0] = jr.g[1] = jr.g[2] = 0.0; jnext = jr;
+#else
+    j2_two_sums<NT>(d, R_s, k, rn, more, rk1, jr, jnext);
+#endif
+    PH(2);
+#ifdef QMC_EXP_KEEP
+    spline_cta<T, NT, NoSideWork, true, true>(d, nullptr, sw, vgl_s);
+#else
+    spline_cta<T, NT, NoSideWork, false, true>(d, nullptr, sw, vgl_s);
+#endif
     __syncthreads();
-    dev_ratio_grad<T, NT>(d, w, k, b_s, vgl_s, R_s, ms, nullptr, nullptr, red);
-    cp_async_wait_all();
-    if (dev_decide(d, w, k, ms, nullptr)) {
+    PH(3);
+    win_ratio_grad<T, NT>(d, b_s, vgl_s, jr, ms, red);   // row dots + block sum; thread 0: rho_D, rho_J, G_k(R')
+    PH(4);
+    // ---- the decision is one thread's scalar chain (two exp, divisions, Philox): the other warps use the time for
+    // what the NEXT move needs and nobody is waiting for -- its Gaussians, the pair term (k+1, k) for both outcomes
+    // ([0..3] rejected, [4..7] accepted), its inverse row (valid unless this move is accepted, which rewrites it) and
+    // its gradient cache ----
+    if (more) {
+      const int warp = tid >> 5, lane = tid & 31;
+      if (warp == 1 % (NT / 32)) {
+        if (lane < 5) gauss[lane] = gauss_piece(d, w, k + 1, lane);
+      }
+      if (warp == 2 % (NT / 32)) {
+        if (lane >= 30) {
+          const bool acc_case = lane == 31;
+          double us = 0.0, g[3] = {0.0, 0.0, 0.0};
+          if (acc_case) j2_pair(d, rk1, rn, us, g);
+          else j2_pair(d, rk1, R_s + 3 * k, us, g);
+          double* o = pairk + (acc_case ? 4 : 0);
+          o[0] = us; o[1] = g[0]; o[2] = g[1]; o[3] = g[2];
+        }
+      }
+      if (warp == 3 % (NT / 32)) {
+        cp_async_warp(bn_s, (m ? Bcur : blk) + (size_t)(i + 1) * ns, row_bytes);
+        cp_async_warp(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
+      }
+    }
+    const int acc_ = dev_decide(d, w, k, ms, nullptr);
+    prev_acc = acc_;
+    PH(5);
+    if (acc_) {
       const double inv_rho = 1.0 / *ms.rho_d;
       for (int j = tid; j < ns; j += NT) {
         const double c = b_s[j] * inv_rho;
@@ -223,13 +414,24 @@ __global__ void __launch_bounds__(NT, 512 / NT) window_kernel(CrowdDev d, int k0
         Rg[3 * k + tid] = x;
       }
       if (tid == 0) rows_s[m] = kk0 + i;
+      cp_async_wait_all();   // the stale copy of the next row has landed before the update overwrites it
       __syncthreads();
+#ifdef QMC_EXP_NOBLOCK
+      block_rows_update<T, NT>(m ? Bcur : blk, Bcur, ns, i + 1, min(cnt, i + 2), vgl_s, b_s, bn_s);
+#else
       block_rows_update<T, NT>(m ? Bcur : blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
+#endif
       ++m;
     }
+    cp_async_wait_all();
     __syncthreads();
+    PH(6);
     double* t = b_s; b_s = bn_s; bn_s = t;
   }
+#ifdef QMC_PHASE_CLOCKS
+  if (tid == 0)
+    for (int q = 0; q < 8; ++q) d.pvec[(size_t)w * kdp + q] += (double)ph_t[q];
+#endif
 
   for (int l = tid; l < m; l += NT) d.rows[(size_t)w * kdp + l] = rows_s[l];
   if (tid == 0) d.mwin[w] = m;
