@@ -48,6 +48,14 @@ struct CrowdDev {
   int* status;                               // [1] != 0: singular matrix met
 };
 
+// Shape accessors of shape-specialised kernels: NS > 0 means n = M = ns = NS and N = 2 NS are compile-time constants
+// (and the table's orbital stride covers ns); NS = 0 reads the crowd's own fields.
+template <int NS> __device__ __forceinline__ int sh_ns(const CrowdDev& d) { return NS > 0 ? NS : d.ns; }
+template <int NS> __device__ __forceinline__ int sh_M(const CrowdDev& d) { return NS > 0 ? NS : d.M; }
+template <int NS> __device__ __forceinline__ int sh_n(const CrowdDev& d) { return NS > 0 ? NS : d.n; }
+template <int NS> __device__ __forceinline__ int sh_N(const CrowdDev& d) { return NS > 0 ? 2 * NS : d.N; }
+template <int NS> __device__ __forceinline__ unsigned sh_tab_vecs(const CrowdDev& d) { return NS > 0 ? 0xffffffffu : d.tab_vecs; }
+
 template <typename T> struct Vec16;
 template <> struct Vec16<float> { static constexpr int W = 4; };
 template <> struct Vec16<double> { static constexpr int W = 2; };

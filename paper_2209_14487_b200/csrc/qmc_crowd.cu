@@ -426,7 +426,13 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   ProfScope ps(c, QMC_K_WINDOW);
   CrowdDev d = c->dev;
   d.w0 = w0;
-  switch (window_threads(d.W)) {   // the class of the WHOLE crowd: a split into sub-crowds never changes a reduction tree
+  const int nt = window_threads(d.W);
+  // shape-specialised instances for the BASELINE.json shapes with n a multiple of 16 (cfgs 3, 4, 5): see window.cuh
+  const bool spec = nt == 128 && sizeof(T) == 4 && d.n == d.ns && d.M == d.n && d.tab_vecs >= (unsigned)d.ns / 4;
+  if (spec && d.ns == 384) window_kernel<T, 128, 384><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt);
+  else if (spec && d.ns == 192) window_kernel<T, 128, 192><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt);
+  else if (spec && d.ns == 96) window_kernel<T, 128, 96><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt);
+  else switch (nt) {   // the class of the WHOLE crowd: a split into sub-crowds never changes a reduction tree
     case 512: window_kernel<T, 512><<<wn, 512, window_smem(d, sizeof(T), 512), st>>>(d, k0, cnt); break;
     case 256: window_kernel<T, 256><<<wn, 256, window_smem(d, sizeof(T), 256), st>>>(d, k0, cnt); break;
     default: window_kernel<T, 128><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt); break;
@@ -451,6 +457,8 @@ cudaError_t raise_smem_limits_t(int optin)
 {
   const void* fns[] = {(const void*)row_propose_kernel<T>, (const void*)ratio_grad_kernel<T>, (const void*)accept_kernel<T>,
                        (const void*)ratio_accept_kernel<T>, (const void*)window_kernel<T, 128>,
+                       (const void*)window_kernel<T, 128, 384>, (const void*)window_kernel<T, 128, 192>,
+                       (const void*)window_kernel<T, 128, 96>,
                        (const void*)window_kernel<T, 256>, (const void*)window_kernel<T, 512>,
                        (const void*)sweep1_kernel<T>, (const void*)spline_build_kernel<T>, (const void*)kinetic_kernel<T>};
   for (const void* f : fns) {

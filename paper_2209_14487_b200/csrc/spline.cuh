@@ -188,7 +188,7 @@ struct NoSideWork { __device__ __forceinline__ void operator()(int) const {} };
 // r == nullptr: the caller has already filled `s` for this position (spline_axis per axis).
 // KEEP: loads without the L2 evict-first hint (callers that arrange for L2 re-use).
 // PRESYNCED: the caller has already synchronised after filling `s` (and may have done work of its own in between).
-template <typename T, int NT, typename Side = NoSideWork, bool KEEP = false, bool PRESYNCED = false>
+template <typename T, int NT, typename Side = NoSideWork, bool KEEP = false, bool PRESYNCED = false, int NS = 0>
 __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, SplineW<T>& s, T* vgl, Side side = Side())
 {
   constexpr int VW = Vec16<T>::W;
@@ -203,12 +203,12 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
     __syncthreads();
   }
   const T* tab = static_cast<const T*>(d.coefs);
-  const unsigned chunks = (unsigned)d.ns / VW;
+  const unsigned chunks = (unsigned)sh_ns<NS>(d) / VW;
 #pragma unroll 1
   for (unsigned c0 = 0; c0 < chunks; c0 += NT / 4) {
     const unsigned chunk = c0 + g;
     T out[5][VW];
-    if (chunk < d.tab_vecs && chunk < chunks) {
+    if (chunk < sh_tab_vecs<NS>(d) && chunk < chunks) {
       T p[4][4][VW];
       spline_plane_load<T, KEEP>(tab, s, a, chunk, p);
       if (c0 == 0 && tid >= 32) side(tid);
@@ -243,31 +243,12 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
     }
 #pragma unroll
     for (int e = 0; e < VW; ++e)
-      if ((int)(chunk * VW) + e >= d.M) f0[e] = f1[e] = (T)0;
+      if ((int)(chunk * VW) + e >= sh_M<NS>(d)) f0[e] = f1[e] = (T)0;
     if (chunk < chunks) {
       T* o = vgl + (size_t)chunk * VW;
-      st16(o + (size_t)a * d.ns, f0);
-      if (a == 0) st16(o + (size_t)4 * d.ns, f1);
+      st16(o + (size_t)a * sh_ns<NS>(d), f0);
+      if (a == 0) st16(o + (size_t)4 * sh_ns<NS>(d), f1);
     }
-  }
-}
-
-// L2 prefetch of the 64 stencil rows of the position whose weights are in `s` (a row = the orbitals of one grid point,
-// contiguous): every thread asks for its share of the rows' 128-byte lines.  prefetch.global.L2 moves DRAM -> L2
-// without occupying a register or a load slot: the gather that follows finds its lines in, or on their way to, L2.
-// (cp.async.bulk.prefetch.L2, one instruction per row, takes its address from a uniform register: ptxas serialises
-// it lane by lane -- 2.5 % of the window kernel's instructions when tried.)
-template <typename T, int NT>
-__device__ __forceinline__ void spline_prefetch_l2(const CrowdDev& d, const SplineW<T>& s)
-{
-  constexpr int VW = Vec16<T>::W;
-  const unsigned vecs = d.tab_vecs < (unsigned)d.ns / VW ? d.tab_vecs : (unsigned)d.ns / VW;
-  const unsigned lines = (vecs + 7) / 8;   // 128-byte lines per row
-  const char* tab = static_cast<const char*>(d.coefs);
-  for (unsigned e = threadIdx.x; e < 64 * lines; e += NT) {
-    const unsigned row = e / lines, ln = e - row * lines;
-    const size_t vec = (size_t)(s.off[0][row >> 4] + s.off[1][(row >> 2) & 3] + s.off[2][row & 3]) + 8 * ln;
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(tab + vec * 16));
   }
 }
 

@@ -81,8 +81,8 @@ __device__ __forceinline__ void cp_async_cta(void* smem, const void* gmem, int n
 // A move needs two pair sums (D:C3): at the current position r_k for G_k(R) (proposal) and at r' for the ratio.  Both
 // are ~70 dependent fp64 instructions per pair, six pairs per thread: next to the row dots they were 2 x 3000 cycles
 // of every move's chain.  Neither depends on what the move itself decides, except through one pair term:
-//   - the sum at r' needs only r' and R: it is evaluated right after the proposal, while the stencil rows of r' are
-//     on their way from DRAM to L2 (spline_prefetch_l2);
+//   - the sum at r' needs only r' and R: it is evaluated right after the proposal, together with the next one, as
+//     straight-line code with four pair chains in flight;
 //   - the sum at r_{k+1} for the NEXT move is evaluated at the same time over all electrons but k (whose position the
 //     pending decision may change); the missing term is evaluated for both outcomes (against r_k and against r'_k)
 //     and the one that applies is added after the decision.
@@ -116,13 +116,13 @@ __device__ __forceinline__ void j2_pair_bf(const CrowdDev& d, const double (&rk)
 // Thread-strided partials of two pair sums at once: electron k placed at rn against all electrons but k, and (if
 // `next`) electron k + 1 at its own position rk1 against all electrons but k and k + 1.  Two electrons per trip, so
 // four independent pair chains are in flight per thread.
-template <int NT>
+template <int NT, int NS = 0>
 __device__ __forceinline__ void j2_two_sums(const CrowdDev& d, const double* R, int k, const double (&rn)[3], bool next,
                                             const double (&rk1)[3], J2Part& at_rn, J2Part& at_next)
 {
   at_rn.us = at_rn.g[0] = at_rn.g[1] = at_rn.g[2] = 0.0;
   at_next.us = at_next.g[0] = at_next.g[1] = at_next.g[2] = 0.0;
-  const int N = d.N;
+  const int N = sh_N<NS>(d);
   for (int i0 = threadIdx.x; i0 < N; i0 += 2 * NT) {
     const int i1 = i0 + NT;
     const bool in1 = i1 < N;
@@ -138,14 +138,14 @@ __device__ __forceinline__ void j2_two_sums(const CrowdDev& d, const double* R, 
 // G_k(R) and the proposal from the row dots and a precomputed Jastrow partial (see dev_gold_propose for the formulas;
 // same products, the pair terms summed in a different order).  extra: the pair term (k, k-1) chosen after the previous
 // decision, added by thread 0 (nullptr for the first move of a window).
-template <typename T, int NT>
+template <typename T, int NT, int NS = 0>
 __device__ __forceinline__ void win_gold_propose(const CrowdDev& d, int k, const double* b_s, const T* cache, const double* R,
                                                  const J2Part& jp, const double* extra, MoveScal ms, double* red,
                                                  const double* gp, SplineW<T>* sw_out)
 {
-  const int ns = d.ns, tid = threadIdx.x;
+  const int ns = sh_ns<NS>(d), tid = threadIdx.x;
   double v[7] = {0.0, 0.0, 0.0, jp.us, jp.g[0], jp.g[1], jp.g[2]};
-  for (int j = tid; j < d.M; j += NT) {
+  for (int j = tid; j < sh_M<NS>(d); j += NT) {
     const double bj = b_s[j];
     v[0] = fma(bj, (double)cache[j], v[0]);
     v[1] = fma(bj, (double)cache[ns + j], v[1]);
@@ -172,13 +172,13 @@ __device__ __forceinline__ void win_gold_propose(const CrowdDev& d, int k, const
 }
 
 // rho_D, rho_J and G_k(R') from the row dots and the precomputed Jastrow partial at r' (see dev_ratio_grad).
-template <typename T, int NT>
+template <typename T, int NT, int NS = 0>
 __device__ __forceinline__ void win_ratio_grad(const CrowdDev& d, const double* b, const T* vgl, const J2Part& jr,
                                                MoveScal ms, double* red)
 {
-  const int ns = d.ns, tid = threadIdx.x;
+  const int ns = sh_ns<NS>(d), tid = threadIdx.x;
   double v[8] = {0.0, 0.0, 0.0, 0.0, jr.us, jr.g[0], jr.g[1], jr.g[2]};
-  for (int j = tid; j < d.M; j += NT) {
+  for (int j = tid; j < sh_M<NS>(d); j += NT) {
     const double bj = b[j];
     v[0] = fma(bj, (double)vgl[j], v[0]);
     v[1] = fma(bj, (double)vgl[ns + j], v[1]);
@@ -285,13 +285,16 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
 #ifndef QMC_WIN_MINCTAS
 #define QMC_WIN_MINCTAS 4
 #endif
-template <typename T, int NT>
+// NS > 0: the kernel is specialised for n = M = ns = NS (N = 2 NS, a table stride that covers ns): every trip count
+// and row stride is a compile-time constant, loops unroll and the index arithmetic folds -- the kernel is bound by its
+// instruction stream, a third of which was integer / control overhead (ncu r2).  NS = 0: any shape.
+template <typename T, int NT, int NS = 0>
 __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) window_kernel(CrowdDev d, int k0, int cnt)
 {
   extern __shared__ double sm[];
   __shared__ SplineW<T> sw;
-  const int w = blockIdx.x + d.w0, ns = d.ns, kdp = d.kdp, tid = threadIdx.x;
-  const WinLayout L = win_layout(d.N, ns, kdp, (int)sizeof(T), NT);
+  const int w = blockIdx.x + d.w0, ns = sh_ns<NS>(d), nN = sh_N<NS>(d), kdp = d.kdp, tid = threadIdx.x;
+  const WinLayout L = win_layout(nN, ns, kdp, (int)sizeof(T), NT);
   double* R_s = sm + L.R;
   double* b_s = sm + L.b;    // row of the current move
   double* bn_s = sm + L.bn;  // row of the next move
@@ -304,20 +307,20 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
   T* vgl_s = reinterpret_cast<T*>(sm + L.vgl);
   const MoveScal ms = move_scal_smem(sm + L.mv);
 
-  const int spin = k0 / d.n, kk0 = k0 - spin * d.n;
+  const int spin = k0 / sh_n<NS>(d), kk0 = k0 - spin * sh_n<NS>(d);
   const double* blk = d.Binv + (((size_t)w * 2 + spin) * ns + kk0) * ns;  // B0 rows of the window
   double* Bcur = d.C + (size_t)w * kdp * ns;                              // their current values, once m > 0
   double* Cp = d.Cp + (size_t)w * kdp * ns;
   double* V = d.V + (size_t)w * kdp * ns;
-  double* Rg = d.R + (size_t)w * d.N * 3;
-  T* cache0 = static_cast<T*>(d.cache) + ((size_t)w * d.N + k0) * 4 * ns;
+  double* Rg = d.R + (size_t)w * nN * 3;
+  T* cache0 = static_cast<T*>(d.cache) + ((size_t)w * nN + k0) * 4 * ns;
   const int row_bytes = ns * 8, cache_bytes = 3 * ns * (int)sizeof(T);
 
   // prologue: row and gradient cache of the first move, positions, Gaussians of the first move;
   // the rest of the block is pulled into L2 (first-touch DRAM lines the first accepted move reads)
   cp_async_cta<NT>(b_s, blk, row_bytes);
   cp_async_cta<NT>(cbuf, cache0, cache_bytes);
-  for (int j = tid; j < 3 * d.N; j += NT) R_s[j] = Rg[j];
+  for (int j = tid; j < 3 * nN; j += NT) R_s[j] = Rg[j];
   if (tid >= 32 && tid < 37) gauss[tid - 32] = gauss_piece(d, w, k0, tid - 32);
   for (int j = tid; j < (cnt - 1) * row_bytes / 128; j += NT)
     asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
@@ -348,29 +351,20 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
     const bool more = i + 1 < cnt;
     PH(0);
     // ---- G_k(R) and the proposal: row dots + the Jastrow partial prepared during the previous move ----
-    win_gold_propose<T, NT>(d, k, b_s, ccur, R_s, jnext, i ? pairk + 4 * prev_acc : nullptr, ms, red, gauss, &sw);
+    win_gold_propose<T, NT, NS>(d, k, b_s, ccur, R_s, jnext, i ? pairk + 4 * prev_acc : nullptr, ms, red, gauss, &sw);
     __syncthreads();   // r' and the spline weights of r' are visible
     PH(1);
-    // ---- stencil rows of r' towards L2; in their shadow both Jastrow sums ----
-    spline_prefetch_l2<T, NT>(d, sw);
+    // ---- both Jastrow sums (at r' for the ratio, at r_{k+1} for the next proposal), four pair chains in flight ----
     J2Part jr;
     const double rn[3] = {ms.rn[0], ms.rn[1], ms.rn[2]};
     const int k1 = more ? k + 1 : k;
     const double rk1[3] = {R_s[3 * k1], R_s[3 * k1 + 1], R_s[3 * k1 + 2]};
-#ifdef QMC_EXP_NOJ2
-    jr.us = jr.g[0] = jr.g[1] = jr.g[2] = 0.0; jnext = jr;
-#else
-    j2_two_sums<NT>(d, R_s, k, rn, more, rk1, jr, jnext);
-#endif
+    j2_two_sums<NT, NS>(d, R_s, k, rn, more, rk1, jr, jnext);
     PH(2);
-#ifdef QMC_EXP_KEEP
-    spline_cta<T, NT, NoSideWork, true, true>(d, nullptr, sw, vgl_s);
-#else
-    spline_cta<T, NT, NoSideWork, false, true>(d, nullptr, sw, vgl_s);
-#endif
+    spline_cta<T, NT, NoSideWork, false, true, NS>(d, nullptr, sw, vgl_s);
     __syncthreads();
     PH(3);
-    win_ratio_grad<T, NT>(d, b_s, vgl_s, jr, ms, red);   // row dots + block sum; thread 0: rho_D, rho_J, G_k(R')
+    win_ratio_grad<T, NT, NS>(d, b_s, vgl_s, jr, ms, red);   // row dots + block sum; thread 0: rho_D, rho_J, G_k(R')
     PH(4);
     // ---- the decision is one thread's scalar chain (two exp, divisions, Philox): the other warps use the time for
     // what the NEXT move needs and nobody is waiting for -- its Gaussians, the pair term (k+1, k) for both outcomes
@@ -416,11 +410,7 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
       if (tid == 0) rows_s[m] = kk0 + i;
       cp_async_wait_all();   // the stale copy of the next row has landed before the update overwrites it
       __syncthreads();
-#ifdef QMC_EXP_NOBLOCK
-      block_rows_update<T, NT>(m ? Bcur : blk, Bcur, ns, i + 1, min(cnt, i + 2), vgl_s, b_s, bn_s);
-#else
       block_rows_update<T, NT>(m ? Bcur : blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
-#endif
       ++m;
     }
     cp_async_wait_all();

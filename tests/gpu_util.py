@@ -91,3 +91,20 @@ class FreeRunningCheck:
 
     def inverse_tol(self, w):
         return 1e-5 if self.departed[w] else 1e-10
+
+
+def straddled_walkers(Ra, Rb, R_before, max_frac=2e-4):
+    """Two CUDA paths that evaluate the same move in different floating-point orders (qmc_sweep's eager-block form and
+    the step calls' bordered form, R5) agree on G to ~1e-12, so they round a displacement to the two different
+    neighbouring fp32 values only where the unrounded value sits on a rounding boundary to that accuracy (reading A7) --
+    in practice a component that cancels to ~1e-6, whose fp32 ulp is ~1e-13.  Positions must be bit-identical except for
+    at most a fraction max_frac of the components, each differing by exactly one fp32 ulp of its own displacement.
+    Returns the walkers that contain such a component (their later moves see inputs that differ by that ulp)."""
+    diff = Ra != Rb
+    if not diff.any():
+        return np.zeros(Ra.shape[0], dtype=bool)
+    assert diff.mean() <= max_frac, f"{diff.sum()} position components differ"
+    delta = np.where(diff, Ra - R_before, 1.0)
+    ulp = np.spacing(np.abs(delta).astype(np.float32)).astype(np.float64)
+    assert (np.abs(Ra - Rb)[diff] <= 1.001 * ulp[diff]).all(), "a position differs by more than one fp32 ulp of its displacement"
+    return diff.any(axis=(1, 2))
