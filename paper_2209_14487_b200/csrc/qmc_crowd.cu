@@ -352,7 +352,7 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     return;
   }
   if (from_window) {
-    flush_finalize_tri_kernel<KDP><<<wn, FINTRI_NT, (size_t)KDP * (KDP + 1) * 8, st>>>(d, 0);
+    if constexpr (KDP <= 32) flush_finalize_tri_kernel<KDP><<<wn, FINTRI_NT, (size_t)KDP * (KDP + 1) * 8, st>>>(d, 0);
   } else {
     const int fcols = FINALIZE_NT / (KDP > 32 ? KDP / 32 : 1);
     dim3 fgrid((d.ns + fcols - 1) / fcols, wn);
