@@ -37,7 +37,7 @@ class System(C.Structure):
     _fields_ = [
         ("n_elec", C.c_int32), ("n_orb", C.c_int32), ("grid", C.c_int32 * 3), ("coef_dtype", C.c_int32),
         ("box", C.c_double * 3), ("coefs", C.c_void_p), ("j2_a", C.c_double), ("j2_b", C.c_double),
-        ("tau", C.c_double), ("seed", C.c_uint64), ("delay_rank", C.c_int32), ("_pad", C.c_int32),
+        ("tau", C.c_double), ("seed", C.c_uint64), ("delay_rank", C.c_int32), ("inverse_fp32", C.c_int32),
     ]
 
 
@@ -80,6 +80,9 @@ def lib():
     L.oracle_crowd_sweep.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
     L.oracle_crowd_sweep.restype = C.c_int64
     L.oracle_crowd_set_sweep_index.argtypes = [C.c_void_p, C.c_uint32]
+    L.oracle_crowd_recompute.argtypes = [C.c_void_p]
+    L.oracle_crowd_recompute.restype = C.c_int
+    L.oracle_round_to_fp32.argtypes = [C.c_int, dp]
     L.oracle_crowd_branch.argtypes = [C.c_void_p, C.c_void_p]
     L.oracle_crowd_branch.restype = C.c_int
     L.oracle_crowd_get_positions.argtypes = [C.c_void_p, dp]
@@ -127,7 +130,7 @@ class OracleSystem:
     """Owns a ``System`` struct and keeps the coefficient array alive."""
 
     def __init__(self, n_elec: int, grid, box, coefs: np.ndarray, j2_a=0.5, j2_b=1.0, tau=0.01,
-                 seed=1, delay_rank=1):
+                 seed=1, delay_rank=1, inverse_fp32=False):
         n_orb = n_elec // 2
         grid = [int(g) for g in grid]
         assert coefs.dtype in (np.float32, np.float64)
@@ -142,6 +145,7 @@ class OracleSystem:
         s.box = (C.c_double * 3)(*self.box)
         s.coefs = self.coefs.ctypes.data
         s.j2_a, s.j2_b, s.tau, s.seed, s.delay_rank = j2_a, j2_b, tau, seed, delay_rank
+        s.inverse_fp32 = 1 if inverse_fp32 else 0
         self.struct = s
 
     @property
@@ -200,6 +204,12 @@ def sm_update(B, k: int, phi, rho_d: float) -> np.ndarray:
     return B
 
 
+def round_to_fp32(B) -> np.ndarray:
+    B = _f64(B).copy()
+    lib().oracle_round_to_fp32(B.shape[0], _dp(B))
+    return B
+
+
 def delayed_row(B0, rows, V, Cm, k: int) -> np.ndarray:
     B0, V, Cm = _f64(B0), _f64(V), _f64(Cm)
     rows = np.ascontiguousarray(rows, dtype=np.int32)
@@ -254,6 +264,11 @@ class OracleCrowd:
 
     def set_sweep_index(self, s: int):
         lib().oracle_crowd_set_sweep_index(self._h, s)
+
+    def recompute(self):
+        st = lib().oracle_crowd_recompute(self._h)
+        if st != 0:
+            raise RuntimeError(f"oracle_crowd_recompute: status {st}")
 
     def branch(self, src):
         src = np.ascontiguousarray(src, dtype=np.int32)

@@ -336,6 +336,13 @@ void oracle_sm_update(int n, double* B, int k, const double* phi, double rho_d)
   free(b_old);
 }
 
+/* R6 (mixed precision): the carried inverse is stored in fp32.  Storage only: the value kept is
+ * the fp32 number nearest to the fp64 result (ties to even: the C conversion), widened again for every later use. */
+void oracle_round_to_fp32(int n, double* B)
+{
+  for (size_t e = 0; e < (size_t)n * n; ++e) B[e] = (double)(float)B[e];
+}
+
 /* C6 (Woodbury): window of m accepted moves since the last flush: rows[l] = electron row
  * replaced by V[l,:] (m x n), C[l,:] = B0[rows[l],:] (m x n), S = V C^T (m x m).
  * Builds S and LU-factors it from scratch (no incremental inverse). */
@@ -515,11 +522,35 @@ oracle_crowd* oracle_crowd_create(const oracle_system* sys, int W, int walker_id
                        c->dphi + ((size_t)w * N + e) * 3 * M, c->d2phi + ((size_t)w * N + e) * M);
       }
       st_all |= oracle_lu_inverse_transpose(n, A, c->B + ((size_t)w * 2 + s) * n * n, NULL, NULL);
+      if (c->sys.inverse_fp32) oracle_round_to_fp32(n, c->B + ((size_t)w * 2 + s) * n * n);
     }
     free(A);
   }
   if (status) *status = st_all;
   return c;
+}
+
+int oracle_crowd_recompute(oracle_crowd* c)
+{
+  const int W = c->W, N = c->N, n = c->n, M = c->M;
+  int st_all = 0;
+  for (int w = 0; w < W; ++w)
+    if (c->m[w] != 0) return -1;
+#pragma omp parallel for schedule(dynamic) reduction(| : st_all)
+  for (int w = 0; w < W; ++w) {
+    double* A = (double*)malloc(sizeof(double) * (size_t)n * n);
+    for (int s = 0; s < 2; ++s) {
+      for (int i = 0; i < n; ++i) {
+        int e = s * n + i;
+        oracle_spo_vgl(&c->sys, c->R + ((size_t)w * N + e) * 3, A + (size_t)i * n,
+                       c->dphi + ((size_t)w * N + e) * 3 * M, c->d2phi + ((size_t)w * N + e) * M);
+      }
+      st_all |= oracle_lu_inverse_transpose(n, A, c->B + ((size_t)w * 2 + s) * n * n, NULL, NULL);
+      if (c->sys.inverse_fp32) oracle_round_to_fp32(n, c->B + ((size_t)w * 2 + s) * n * n);
+    }
+    free(A);
+  }
+  return st_all;
 }
 
 /* One sweep (k = 0..N-1) of one walker: Alg. 1 lines 4-9, steps a0..a5
@@ -590,11 +621,13 @@ static int64_t walker_sweep(oracle_crowd* c, int w, uint32_t s, oracle_move_log*
         ++*mw;
       } else {                /* a4: rank-1 */
         oracle_sm_update(n, B, kk, phi, rho_d);
+        if (sys->inverse_fp32) oracle_round_to_fp32(n, B);   /* R6: stored in fp32 */
       }
     }
     /* a5: flush after every kd PROPOSED moves of a spin block and at its end (C6 schedule) */
     if (kd > 1 && (((kk + 1) % kd) == 0 || kk == n - 1)) {
       oracle_delayed_flush(n, B, *mw, rows, V, C);
+      if (sys->inverse_fp32 && *mw > 0) oracle_round_to_fp32(n, B);   /* R6: stored in fp32 */
       *mw = 0;
     }
     if (log) log[k] = rec;

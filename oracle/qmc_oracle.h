@@ -29,6 +29,9 @@
  *   SM / delayed .. full re-inversion (numpy) after every accepted move / flush
  *   Jastrow ....... two-electron closed form, full pair-sum difference, finite differences
  *   accept rule ... tau->0 limit, constant-orbital case, sampling of |phi|^2 (histogram)
+ *   fp32 storage .. (mixed precision, R6) every stored element is its own fp32 rounding; with fp32-representable
+ *                   inputs one update equals the fp64 update rounded once; the carried inverse stays within the
+ *                   first-order bound r kappa_inf(A) 2^-24 of the exact one (tests/test_oracle_mixed.py)
  *   kinetic ....... central second differences of the brute-force Psi = det det exp(J) (numpy) on tiny systems;
  *                   free-particle and two-electron Jastrow closed forms
  *   whole sweep ... every logged move re-derived from brute-force determinants; the
@@ -55,7 +58,10 @@ typedef struct {
   double  tau;         /* time step                                                        */
   uint64_t seed;       /* Philox key                                                       */
   int32_t delay_rank;  /* 1 = Sherman-Morrison, k > 1 = delayed rank-k                     */
-  int32_t _pad;
+  int32_t inverse_fp32;/* 0: the carried inverse is fp64 (BASELINE.json configs).  1: mixed precision (SURVEY.md 8(f)
+                          item 3, reading R6): the carried inverse is STORED in fp32 -- every element is rounded
+                          to the nearest fp32 value after each operation that writes it (inversion, rank-1 update,
+                          flush) -- while every dot product and update is evaluated in fp64 on the stored values      */
 } oracle_system;
 
 /* one record per (walker, electron) move of a sweep; everything the acceptance needs */
@@ -116,6 +122,12 @@ void oracle_crowd_destroy(oracle_crowd* c);
  * [n_sweeps][W][N] records. Returns number of accepted moves. Threads over walkers. */
 int64_t oracle_crowd_sweep(oracle_crowd* c, int n_sweeps, oracle_move_log* log);
 void oracle_crowd_set_sweep_index(oracle_crowd* c, uint32_t s);
+/* periodic recompute: rebuilds both Slater matrices from the carried positions, inverts
+ * them by LU in fp64 (then rounds to fp32 in the mixed-precision mode) and refreshes the caches; needs an empty
+ * window.  Returns the LU status (0 = ok), -1 on an open window. */
+int  oracle_crowd_recompute(oracle_crowd* c);
+/* R6: x <- fl32(x) for the n x n carried inverse (round to nearest even, the C cast) */
+void oracle_round_to_fp32(int n, double* B);
 /* branching data movement: slot w <- state of slot src[w]; -1 on a bad entry / open window */
 int  oracle_crowd_branch(oracle_crowd* c, const int32_t* src /*[W]*/);
 void oracle_crowd_get_positions(const oracle_crowd* c, double* pos /*[W][N][3]*/);
