@@ -227,12 +227,12 @@ def algorithmic(wl, W, kd, alpha, el, m_move=None):
 # ----------------------------------------------------------------------------------------------
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------
-def make_crowd(wl, W, kd, id0, coefs_dev, dev):
+def make_crowd(wl, W, kd, id0, coefs_dev, dev, inverse_fp32=False):
     import torch
     import paper_2209_14487_b200 as q
     pos = qi.make_positions(wl, id0 + W)[id0:]
     return q.Crowd(coefs_dev, wl.box, torch.from_numpy(np.ascontiguousarray(pos)).to(dev), tau=wl.tau, delay_rank=kd,
-                   j2_a=wl.j2_a, j2_b=wl.j2_b, seed=wl.seed, walker_id0=id0), pos
+                   j2_a=wl.j2_a, j2_b=wl.j2_b, seed=wl.seed, walker_id0=id0, inverse_fp32=inverse_fp32), pos
 
 
 def time_sweeps(crowd, steps, warmup, sync_all):
@@ -523,6 +523,17 @@ def run_cuda(args):
                                                   "avg_us": kernels[name]["avg_us"],
                                                   "share_of_step": kernels[name]["share"]}, name)
 
+    if dom == "flush" and "flush" in extra_rooflines:
+        # the DMMA flush has the largest share of the step: it is the dominant kernel, bound by the FP64 tensor pipe;
+        # the window kernel's HBM roofline moves to rooflines["window"]
+        extra_rooflines["window"] = with_traffic({
+            "kernel": "window", "bound": "hbm", "achieved": kernels["window"]["gbs"], "peak": pk["hbm_gbs"],
+            "unit": "GB/s", "frac": kernels["window"]["gbs"] / pk["hbm_gbs"], "peak_source": pk["source"] + ", of measured",
+            "share_of_step": kernels["window"]["share"], "avg_us": kernels["window"]["avg_us"],
+            "algorithmic_bytes_per_launch": alg["window"]["bytes"], "bytes_counted": "compulsory HBM bytes (DESIGN.md section 6)",
+            "l2_plus_hbm_bytes": alg["window"]["l2_plus_hbm_bytes"]}, "window") if "window" in kernels else None
+        roofline = dict(extra_rooflines["flush"])
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -598,6 +609,22 @@ def run_cuda(args):
             del c2
             torch.cuda.empty_cache()
         line["crowd_sweep"] = sorted(sweep_pts, key=lambda r: (r["delay_rank"], r["walkers"]))
+
+    if rank == 0 and world == 1 and not args.no_sweep_points and kd <= 32:
+        # Mixed precision (R6): the same workload with the carried inverses STORED in
+        # fp32 (all arithmetic fp64).  An extra number, never the headline: BASELINE.json's configs say fp64 inverses.
+        c3, _ = make_crowd(wl, W, kd, 0, coefs_dev, dev, inverse_fp32=True)
+        ms3, prop3, acc3, _ = time_sweeps(c3, 2, 1, torch.cuda.synchronize)
+        c3.set_option(q.QMC_OPT_PROFILE, 1)
+        c3.qmc_sweep(1)
+        p3 = c3.profile()
+        line["mixed_precision"] = {"dtype": "f32inv", "what": "inverses stored in fp32, fp64 arithmetic (DESIGN.md R6)",
+                                   "value": prop3 / (ms3 * 1e-3), "unit": UNIT, "ms_per_sweep": ms3 / 2,
+                                   "accept_fraction": acc3 / prop3,
+                                   "kernels_avg_us": {k2: 1e3 * v[0] / v[1] for k2, v in p3.items() if v[1]}}
+        c3.close()
+        del c3
+        torch.cuda.empty_cache()
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = len(os.sched_getaffinity(0))

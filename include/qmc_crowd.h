@@ -63,7 +63,13 @@ typedef struct {
   int32_t walker_id0;  /* global id of walker 0: Philox counter word 0 is walker_id0 + w (D:C7), */
                        /* so splitting a population into crowds does not change any trajectory   */
   int32_t delay_rank;  /* 1 = Sherman-Morrison rank-1 (D:C5); 2..64 = delayed rank-k (D:C6)      */
-  int32_t _pad;
+  int32_t inverse_dtype; /* 0 = the carried inverses are fp64 (BASELINE.json configs).  1 = mixed    */
+                       /* precision (SURVEY 8(f) item 3, D:R6): the carried inverses are STORED in  */
+                       /* fp32 -- rounded to nearest after every operation that writes them         */
+                       /* (inversion, rank-1 update, flush) -- and every dot product and update is  */
+                       /* evaluated in fp64 on the stored values; halves the dominant bytes of the  */
+                       /* update kernels.  Needs delay_rank <= 32 (a flush is then ONE pass, one    */
+                       /* rounding).  Companion: QMC_OPT_RECOMPUTE_EVERY (fp64 re-inversion).       */
   uint64_t seed;       /* Philox key (lo, hi)                                                    */
   void* workspace;     /* DEVICE, BORROWED, 256-byte aligned                                     */
   size_t workspace_bytes; /* >= qmc_crowd_workspace_bytes(&desc)                                 */

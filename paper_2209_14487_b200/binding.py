@@ -42,7 +42,7 @@ class CrowdDesc(C.Structure):
         ("n_elec", C.c_int32), ("n_orb", C.c_int32), ("grid", C.c_int32 * 3), ("coef_dtype", C.c_int32),
         ("box", C.c_double * 3), ("coefs", C.c_void_p), ("orb_stride", C.c_int64),
         ("j2_a", C.c_double), ("j2_b", C.c_double), ("tau", C.c_double),
-        ("n_walkers", C.c_int32), ("walker_id0", C.c_int32), ("delay_rank", C.c_int32), ("_pad", C.c_int32),
+        ("n_walkers", C.c_int32), ("walker_id0", C.c_int32), ("delay_rank", C.c_int32), ("inverse_dtype", C.c_int32),
         ("seed", C.c_uint64), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p),
     ]
 
@@ -119,7 +119,7 @@ class Crowd:
     """A crowd of walkers advanced in lock-step.  Methods carry the C names."""
 
     def __init__(self, coefs, box, positions, *, tau, delay_rank=1, j2_a=0.5, j2_b=1.0, seed=1, walker_id0=0,
-                 n_orb=None, stream=None):
+                 n_orb=None, stream=None, inverse_fp32=False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("qmc crowd needs a CUDA device; there is no CPU fallback")
@@ -147,6 +147,7 @@ class Crowd:
         d.orb_stride = coefs.shape[3]
         d.j2_a, d.j2_b, d.tau = j2_a, j2_b, tau
         d.n_walkers, d.walker_id0, d.delay_rank = W, walker_id0, delay_rank
+        d.inverse_dtype = 1 if inverse_fp32 else 0
         d.seed = seed
         d.stream = self.stream.cuda_stream
         need = L.qmc_crowd_workspace_bytes(C.byref(d))

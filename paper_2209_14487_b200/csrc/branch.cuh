@@ -53,7 +53,8 @@ struct WalkerState {
 };
 __host__ __device__ inline WalkerState walker_state(const CrowdDev& d, size_t elem)
 {
-  return WalkerState{(size_t)2 * d.ns * d.ns * 8, (size_t)d.N * 4 * d.ns * elem, (size_t)d.N * 3 * 8};
+  // the carried inverses in their storage type (fp64, or fp32 in the mixed-precision mode D:R6)
+  return WalkerState{(size_t)2 * d.ns * d.ns * (d.Binv32 ? 4 : 8), (size_t)d.N * 4 * d.ns * elem, (size_t)d.N * 3 * 8};
 }
 
 // grid = (chunks, W): CTA (c, w) copies its share of the three state arrays of walker src[w] into walker w
@@ -62,7 +63,8 @@ __global__ void __launch_bounds__(BRANCH_NT) branch_copy_kernel(CrowdDev d, cons
   const int w = blockIdx.y, s = src[w];
   if (s == w) return;
   const unsigned long long pol = l2_evict_first_policy();
-  stream_copy16(d.Binv + (size_t)w * (ws.inv_bytes / 8), d.Binv + (size_t)s * (ws.inv_bytes / 8), ws.inv_bytes / 16, pol);
+  double* inv = d.Binv32 ? reinterpret_cast<double*>(d.Binv32) : d.Binv;
+  stream_copy16(inv + (size_t)w * (ws.inv_bytes / 8), inv + (size_t)s * (ws.inv_bytes / 8), ws.inv_bytes / 16, pol);
   stream_copy16(reinterpret_cast<double*>(static_cast<char*>(d.cache) + (size_t)w * ws.cache_bytes),
                 reinterpret_cast<const double*>(static_cast<const char*>(d.cache) + (size_t)s * ws.cache_bytes),
                 ws.cache_bytes / 16, pol);
@@ -80,7 +82,7 @@ __global__ void __launch_bounds__(BRANCH_NT) walker_pack_kernel(CrowdDev d, cons
   double* b_inv = reinterpret_cast<double*>(buf + (size_t)i * ws.total());
   double* b_cache = reinterpret_cast<double*>(buf + (size_t)i * ws.total() + ws.inv_bytes);
   double* b_pos = reinterpret_cast<double*>(buf + (size_t)i * ws.total() + ws.inv_bytes + ws.cache_bytes);
-  double* w_inv = d.Binv + (size_t)w * (ws.inv_bytes / 8);
+  double* w_inv = (d.Binv32 ? reinterpret_cast<double*>(d.Binv32) : d.Binv) + (size_t)w * (ws.inv_bytes / 8);
   double* w_cache = reinterpret_cast<double*>(static_cast<char*>(d.cache) + (size_t)w * ws.cache_bytes);
   double* w_pos = d.R + (size_t)w * (ws.pos_bytes / 8);
   if (EXPORT) {

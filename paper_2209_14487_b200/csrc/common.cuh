@@ -3,6 +3,7 @@
 // Layout of the caller-owned workspace:
 //   R      fp64 [W][N][3]          positions, not wrapped (D:C1)
 //   Binv   fp64 [W][2][ns][ns]     B = (A^-1)^T per spin, row = electron (D:A9); ns = n rounded
+//                                  (mixed precision, D:R6: carried as fp32 in Binv32 [W][2][ns][ns])
 //                                  up to 16, padding rows/columns are zero and stay zero
 //   cache  T    [W][N][4][ns]      d/dx, d/dy, d/dz, laplacian of phi at the electron's current
 //                                  position (D:A12, A13); T = table type
@@ -32,6 +33,8 @@ struct CrowdDev {
   const void* coefs;
   double* R;
   double* Binv;
+  float* Binv32;  // mixed precision (D:R6): the carried inverses, stored in fp32 [W][2][ns][ns]; Binv is then the
+                  // fp64 scratch of the (re)inversion.  nullptr: the inverses are carried in Binv
   void* cache;
   void* vgl;
   double* brow;
@@ -55,6 +58,13 @@ template <int NS> __device__ __forceinline__ int sh_M(const CrowdDev& d) { retur
 template <int NS> __device__ __forceinline__ int sh_n(const CrowdDev& d) { return NS > 0 ? NS : d.n; }
 template <int NS> __device__ __forceinline__ int sh_N(const CrowdDev& d) { return NS > 0 ? 2 * NS : d.N; }
 template <int NS> __device__ __forceinline__ unsigned sh_tab_vecs(const CrowdDev& d) { return NS > 0 ? 0xffffffffu : d.tab_vecs; }
+
+// Row i of the carried inverse of (walker, spin): read where it is stored, widened to fp64 (non-hot kernels; the hot
+// kernels are templated on the storage type).
+__device__ __forceinline__ double ld_binv(const CrowdDev& d, size_t idx)
+{
+  return d.Binv32 ? (double)d.Binv32[idx] : d.Binv[idx];
+}
 
 template <typename T> struct Vec16;
 template <> struct Vec16<float> { static constexpr int W = 4; };

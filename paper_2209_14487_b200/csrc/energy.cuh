@@ -31,13 +31,13 @@ __global__ void __launch_bounds__(EKIN_NT) kinetic_kernel(CrowdDev d, double* __
   const int k_end = min((int)(blockIdx.x + 1) * EKIN_EPB, d.N);
   for (int k = blockIdx.x * EKIN_EPB + warp; k < k_end; k += EKIN_NT / 32) {
     const int spin = k / d.n, kk = k - spin * d.n;
-    const double* b = d.Binv + (((size_t)w * 2 + spin) * ns + kk) * ns;
+    const size_t b = (((size_t)w * 2 + spin) * ns + kk) * ns;   // the electron's inverse row, fp64 or fp32 storage
     const T* cache = static_cast<const T*>(d.cache) + ((size_t)w * d.N + k) * 4 * ns;
     // v[0..2] = b.grad phi, v[3] = b.lap phi, v[4..6] = grad_k J, v[7] = lap_k J
     double v[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll 4   // 20 independent loads in flight per lane (the loop is otherwise one L2 round trip per iteration)
     for (int j = lane; j < d.M; j += 32) {
-      const double bj = b[j];
+      const double bj = ld_binv(d, b + j);
       v[0] = fma(bj, (double)cache[j], v[0]);
       v[1] = fma(bj, (double)cache[ns + j], v[1]);
       v[2] = fma(bj, (double)cache[2 * ns + j], v[2]);

@@ -367,6 +367,15 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
   }
 }
 
+// D:R6: dst = fl32(src), four elements per thread (total % 4 == 0: ns is a multiple of 16)
+__global__ void __launch_bounds__(256) narrow_kernel(float* __restrict__ dst, const double* __restrict__ src, size_t total)
+{
+  for (size_t e = ((size_t)blockIdx.x * 256 + threadIdx.x) * 4; e < total; e += (size_t)gridDim.x * 256 * 4) {
+    const double2 a = *reinterpret_cast<const double2*>(src + e), b = *reinterpret_cast<const double2*>(src + e + 2);
+    *reinterpret_cast<float4*>(dst + e) = make_float4((float)a.x, (float)a.y, (float)b.x, (float)b.y);
+  }
+}
+
 // dst[(b * rows + r) * cols + c] = src[b * sb + r * sr + c]   (gather = pack; scatter = unpack)
 template <typename TD, typename TS>
 __global__ void pack_kernel(TD* __restrict__ dst, const TS* __restrict__ src, size_t nb, int rows, int cols, size_t sb,

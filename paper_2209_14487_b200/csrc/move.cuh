@@ -333,10 +333,10 @@ __device__ __forceinline__ void dev_row_propose(const CrowdDev& d, int w, int k,
   double* y_s = p_s + kdp;
   double* red = y_s + kdp;
   const int spin = k / d.n, kk = k - spin * d.n;
-  const double* B0 = d.Binv + ((size_t)w * 2 + spin) * ns * ns;
+  const size_t B0 = ((size_t)w * 2 + spin) * ns * ns;   // index of the matrix in the carried inverses (fp64 or fp32 storage)
   const int m = d.kd > 1 ? d.mwin[w] : 0;
 
-  for (int j = tid; j < ns; j += MOVE_NT) b_s[j] = B0[(size_t)kk * ns + j];
+  for (int j = tid; j < ns; j += MOVE_NT) b_s[j] = ld_binv(d, B0 + (size_t)kk * ns + j);
   __syncthreads();
   if (m > 0) {
     const double* V = d.V + (size_t)w * kdp * ns;
@@ -379,7 +379,7 @@ __device__ __forceinline__ void dev_accept_update(const CrowdDev& d, int w, int 
   const int m = d.mwin[w];
   double* V = d.V + (size_t)w * kdp * ns;
   double* C = d.C + (size_t)w * kdp * ns;
-  const double* B0k = d.Binv + (((size_t)w * 2 + spin) * ns + kk) * ns;
+  const size_t B0k = (((size_t)w * 2 + spin) * ns + kk) * ns;
   double* q_s = sm;            // [kdp]  q_l = C[l,:].phi'
   double* z_s = q_s + kdp;     // [kdp]  z = q^T Sinv
   double* y_s = z_s + kdp;     // [kdp]  y = Sinv p
@@ -389,7 +389,7 @@ __device__ __forceinline__ void dev_accept_update(const CrowdDev& d, int w, int 
     const double ph = (double)vgl[j];
     phi_s[j] = ph;
     V[(size_t)m * ns + j] = ph;
-    C[(size_t)m * ns + j] = B0k[j];
+    C[(size_t)m * ns + j] = ld_binv(d, B0k + j);
   }
   for (int l = tid; l < m; l += MOVE_NT) y_s[l] = d.yvec[(size_t)w * kdp + l];
   __syncthreads();

@@ -4,6 +4,7 @@
 // spline.cuh / move.cuh / update.cuh / invert.cuh; there is no CPU fallback.
 #include "../../include/qmc_crowd.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -133,6 +134,7 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
   };
   char* R = take(W * N * 3 * 8);
   char* Binv = take(W * 2 * ns * ns * 8);
+  char* Binv32 = ds->inverse_dtype ? take(W * 2 * ns * ns * 4) : nullptr;
   char* cache = take(W * N * 4 * ns * el);
   char* vgl = take(W * 5 * ns * el);
   char* brow = take(W * ns * 8);
@@ -162,7 +164,7 @@ size_t carve(const qmc_crowd_desc* ds, CrowdDev* d, char* base)
   const size_t cells = (size_t)ds->grid[0] * ds->grid[1] * ds->grid[2];
   char* cell_bins = cells <= ((size_t)1 << 22) ? take((cells + 1) * 4) : nullptr;   // Slater build in grid-cell order
   if (d) {
-    d->R = (double*)R; d->Binv = (double*)Binv; d->cache = cache; d->vgl = vgl; d->brow = (double*)brow;
+    d->R = (double*)R; d->Binv = (double*)Binv; d->Binv32 = (float*)Binv32; d->cache = cache; d->vgl = vgl; d->brow = (double*)brow;
     d->rnew = (double*)rnew; d->delta = (double*)delta; d->g_old = (double*)g_old; d->g_new = (double*)g_new;
     d->usum_old = (double*)usum_old; d->rho_d = (double*)rho_d; d->rho_j = (double*)rho_j;
     d->p = (double*)p; d->u = (double*)u; d->accepted = (unsigned char*)accepted;
@@ -186,6 +188,9 @@ int check_desc(const qmc_crowd_desc* ds)
   if (ds->n_walkers > 32767) return fail(QMC_ERR_INVALID_ARG, "n_walkers must be <= 32767 per crowd (split the population into crowds)");
   if (ds->coef_dtype != 0 && ds->coef_dtype != 1) return fail(QMC_ERR_INVALID_ARG, "coef_dtype must be 0 or 1");
   if (ds->delay_rank < 1 || ds->delay_rank > 64) return fail(QMC_ERR_INVALID_ARG, "delay_rank must be in [1,64]");
+  if (ds->inverse_dtype != 0 && ds->inverse_dtype != 1) return fail(QMC_ERR_INVALID_ARG, "inverse_dtype must be 0 (fp64) or 1 (fp32 storage)");
+  if (ds->inverse_dtype == 1 && ds->delay_rank > 32)
+    return fail(QMC_ERR_INVALID_ARG, "fp32-stored inverses need delay_rank <= 32 (one flush pass = one rounding)");
   const int vw = ds->coef_dtype ? 2 : 4;
   if (ds->orb_stride < ds->n_orb || ds->orb_stride % vw) return fail(QMC_ERR_INVALID_ARG, "orb_stride must be >= n_orb and a multiple of %d", vw);
   double tab = (double)ds->orb_stride / vw;
@@ -257,6 +262,11 @@ int rebuild(qmc_crowd* c)
     invert_kernel<<<(unsigned)(d.W * 2), INV_NT, smem, c->stream>>>(d);
   }
   LAUNCH_CHECK(c);
+  if (d.Binv32) {   // D:R6: the fp64 inverse is rounded once into the carried fp32 copy
+    const size_t total = (size_t)d.W * 2 * d.ns * d.ns;
+    narrow_kernel<<<(unsigned)std::min<size_t>((total / 4 + 255) / 256, 148 * 32), 256, 0, c->stream>>>(d.Binv32, d.Binv, total);
+    LAUNCH_CHECK(c);
+  }
   int status = 0;
   CUDA_TRY(cudaMemcpyAsync(&status, d.status, 4, cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(cudaStreamSynchronize(c->stream));
@@ -306,6 +316,11 @@ int launch_rank1_t(qmc_crowd* c, int k)
   const int rows_per_cta = (RANK1_NT / 32) * RANK1_ROWS_PER_WARP;
   dim3 grid((d.n + rows_per_cta - 1) / rows_per_cta, d.W);
   const int nv = (d.ns + 63) / 64;
+  if (d.Binv32) {
+    rank1_f32_kernel<T><<<grid, RANK1_NT, 0, c->stream>>>(d, k);
+    LAUNCH_CHECK(c);
+    return QMC_OK;
+  }
   switch (nv) {
     case 1: rank1_kernel<T, 1><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
     case 2: rank1_kernel<T, 2><<<grid, RANK1_NT, 0, c->stream>>>(d, k); break;
@@ -358,7 +373,8 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     dim3 fgrid((d.ns + fcols - 1) / fcols, wn);
     flush_finalize_kernel<KDP><<<fgrid, FINALIZE_NT, (size_t)KDP * KDP * 8, st>>>(d, spin);
   }
-  flush_kernel<KDP / 8><<<grid, FLUSH_NT, 0, st>>>(d, spin);
+  if (d.Binv32) flush_kernel<KDP / 8, -1, float><<<grid, FLUSH_NT, 0, st>>>(d, spin);   // D:R6, delay_rank <= 32: one pass
+  else flush_kernel<KDP / 8><<<grid, FLUSH_NT, 0, st>>>(d, spin);
 }
 
 // Flush of walkers [w0, w0 + wn) on stream st (the whole crowd on the crowd's stream by default).
@@ -427,15 +443,21 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   CrowdDev d = c->dev;
   d.w0 = w0;
   const int nt = window_threads(d.W);
+  const size_t smem = window_smem(d, sizeof(T), nt);
   // shape-specialised instances for the BASELINE.json shapes with n a multiple of 16 (cfgs 3, 4, 5): see window.cuh
   const bool spec = nt == 128 && sizeof(T) == 4 && d.n == d.ns && d.M == d.n && d.tab_vecs >= (unsigned)d.ns / 4;
-  if (spec && d.ns == 384) window_kernel<T, 128, 384><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt);
-  else if (spec && d.ns == 192) window_kernel<T, 128, 192><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt);
-  else if (spec && d.ns == 96) window_kernel<T, 128, 96><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt);
+  if (d.Binv32) {   // mixed precision (D:R6): the block's B0 rows are fp32
+    if (spec && d.ns == 384) window_kernel<T, 128, 384, float><<<wn, 128, smem, st>>>(d, k0, cnt);
+    else if (nt == 512) window_kernel<T, 512, 0, float><<<wn, 512, smem, st>>>(d, k0, cnt);
+    else if (nt == 256) window_kernel<T, 256, 0, float><<<wn, 256, smem, st>>>(d, k0, cnt);
+    else window_kernel<T, 128, 0, float><<<wn, 128, smem, st>>>(d, k0, cnt);
+  } else if (spec && d.ns == 384) window_kernel<T, 128, 384><<<wn, 128, smem, st>>>(d, k0, cnt);
+  else if (spec && d.ns == 192) window_kernel<T, 128, 192><<<wn, 128, smem, st>>>(d, k0, cnt);
+  else if (spec && d.ns == 96) window_kernel<T, 128, 96><<<wn, 128, smem, st>>>(d, k0, cnt);
   else switch (nt) {   // the class of the WHOLE crowd: a split into sub-crowds never changes a reduction tree
-    case 512: window_kernel<T, 512><<<wn, 512, window_smem(d, sizeof(T), 512), st>>>(d, k0, cnt); break;
-    case 256: window_kernel<T, 256><<<wn, 256, window_smem(d, sizeof(T), 256), st>>>(d, k0, cnt); break;
-    default: window_kernel<T, 128><<<wn, 128, window_smem(d, sizeof(T), 128), st>>>(d, k0, cnt); break;
+    case 512: window_kernel<T, 512><<<wn, 512, smem, st>>>(d, k0, cnt); break;
+    case 256: window_kernel<T, 256><<<wn, 256, smem, st>>>(d, k0, cnt); break;
+    default: window_kernel<T, 128><<<wn, 128, smem, st>>>(d, k0, cnt); break;
   }
   LAUNCH_CHECK(c);
   return QMC_OK;
@@ -458,7 +480,9 @@ cudaError_t raise_smem_limits_t(int optin)
   const void* fns[] = {(const void*)row_propose_kernel<T>, (const void*)ratio_grad_kernel<T>, (const void*)accept_kernel<T>,
                        (const void*)ratio_accept_kernel<T>, (const void*)window_kernel<T, 128>,
                        (const void*)window_kernel<T, 128, 384>, (const void*)window_kernel<T, 128, 192>,
-                       (const void*)window_kernel<T, 128, 96>,
+                       (const void*)window_kernel<T, 128, 96>, (const void*)window_kernel<T, 128, 384, float>,
+                       (const void*)window_kernel<T, 128, 0, float>, (const void*)window_kernel<T, 256, 0, float>,
+                       (const void*)window_kernel<T, 512, 0, float>,
                        (const void*)window_kernel<T, 256>, (const void*)window_kernel<T, 512>,
                        (const void*)sweep1_kernel<T>, (const void*)spline_build_kernel<T>, (const void*)kinetic_kernel<T>};
   for (const void* f : fns) {
@@ -529,7 +553,7 @@ int sweep_once(qmc_crowd* c)
     LAUNCH_CHECK(c);
     return QMC_OK;
   }
-  if (d.ns <= SWEEP1_MAX_NS) {
+  if (d.ns <= SWEEP1_MAX_NS && !d.Binv32) {
     // small matrices: the whole sweep in one walker-persistent launch (window.cuh, sweep1_kernel)
     ProfScope ps(c, QMC_K_WINDOW);
     if (c->is_f64) sweep1_kernel<double><<<d.W, MOVE_NT, window_smem(d, 8), c->stream>>>(d);
@@ -866,7 +890,8 @@ int qmc_crowd_get_inverse(qmc_crowd_t* c, int spin, double* binv_dev)
   if (!c || !binv_dev || spin < 0 || spin > 1) return fail(QMC_ERR_INVALID_ARG, "bad argument");
   const CrowdDev& d = c->dev;
   const size_t ns = (size_t)d.ns;
-  int st = launch_pack(c, binv_dev, d.Binv + (size_t)spin * ns * ns, d.W, d.n, d.n, 2 * ns * ns, ns, 0);
+  int st = d.Binv32 ? launch_pack(c, binv_dev, d.Binv32 + (size_t)spin * ns * ns, d.W, d.n, d.n, 2 * ns * ns, ns, 0)
+                    : launch_pack(c, binv_dev, d.Binv + (size_t)spin * ns * ns, d.W, d.n, d.n, 2 * ns * ns, ns, 0);
   if (st) return st;
   CUDA_TRY(cudaStreamSynchronize(c->stream));
   return QMC_OK;
@@ -878,7 +903,8 @@ int qmc_crowd_set_inverse(qmc_crowd_t* c, int spin, const double* binv_dev)
   if (c->state != ST_IDLE || !c->win_rows.empty()) return fail(QMC_ERR_STATE, "set_inverse needs an empty window");
   const CrowdDev& d = c->dev;
   const size_t ns = (size_t)d.ns;
-  int st = launch_pack(c, d.Binv + (size_t)spin * ns * ns, binv_dev, d.W, d.n, d.n, 2 * ns * ns, ns, 1);
+  int st = d.Binv32 ? launch_pack(c, d.Binv32 + (size_t)spin * ns * ns, binv_dev, d.W, d.n, d.n, 2 * ns * ns, ns, 1)
+                    : launch_pack(c, d.Binv + (size_t)spin * ns * ns, binv_dev, d.W, d.n, d.n, 2 * ns * ns, ns, 1);
   if (st) return st;
   CUDA_TRY(cudaStreamSynchronize(c->stream));
   return QMC_OK;

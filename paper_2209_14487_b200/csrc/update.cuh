@@ -102,6 +102,40 @@ __global__ void __launch_bounds__(RANK1_NT) rank1_generic_kernel(CrowdDev d, int
   }
 }
 
+// Mixed precision (D:R6): the same update on fp32-stored rows -- widened on load, updated in fp64, rounded once on store
+// (8 n^2 bytes per accepted walker-move).  Two passes over the row (the second one hits L1).
+template <typename T>
+__global__ void __launch_bounds__(RANK1_NT) rank1_f32_kernel(CrowdDev d, int k)
+{
+  const int w = blockIdx.y;
+  if (!d.accepted[w]) return;
+  const int ns = d.ns, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int spin = k / d.n, kk = k - spin * d.n;
+  float* B = d.Binv32 + ((size_t)w * 2 + spin) * ns * ns;
+  const double* bo = d.brow + (size_t)w * ns;
+  const T* phi = static_cast<const T*>(d.vgl) + (size_t)w * 5 * ns;
+  const double inv_rho = 1.0 / d.rho_d[w];
+  const int row0 = (blockIdx.x * (RANK1_NT / 32) + warp) * RANK1_ROWS_PER_WARP;
+  for (int rr = 0; rr < RANK1_ROWS_PER_WARP; ++rr) {
+    const int i = row0 + rr;
+    if (i >= d.n) break;
+    float2* row = reinterpret_cast<float2*>(B + (size_t)i * ns);
+    double acc = 0.0;
+    for (int jj = lane; jj < ns / 2; jj += 32) {   // same lane partition and order as rank1_kernel
+      const float2 x = row[jj];
+      acc = fma((double)x.x, (double)phi[2 * jj], acc);
+      acc = fma((double)x.y, (double)phi[2 * jj + 1], acc);
+    }
+    acc = warp_sum(acc);
+    const double f = (acc - (i == kk ? 1.0 : 0.0)) * inv_rho;
+    for (int jj = lane; jj < ns / 2; jj += 32) {
+      const float2 x = row[jj];
+      const double2 b2 = *reinterpret_cast<const double2*>(bo + 2 * jj);
+      row[jj] = make_float2((float)fma(-f, b2.x, (double)x.x), (float)fma(-f, b2.y, (double)x.y));
+    }
+  }
+}
+
 #ifndef QMC_FLUSH_MIN_CTAS
 #define QMC_FLUSH_MIN_CTAS 3
 #endif
@@ -122,6 +156,24 @@ __device__ __forceinline__ void st32(double* p, double a, double b, double c, do
 {
   asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
 }
+
+// Four consecutive elements of the carried inverse in its storage type (D:R6): fp64, or fp32 widened on load and
+// rounded to nearest on store.
+__device__ __forceinline__ void ld_b4(const double* p, double (&v)[4]) { ld32(p, v); }
+__device__ __forceinline__ void ld_b4(const float* p, double (&v)[4])
+{
+  float4 f;
+  asm volatile("ld.global.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(f.x), "=f"(f.y), "=f"(f.z), "=f"(f.w) : "l"(p));
+  v[0] = (double)f.x; v[1] = (double)f.y; v[2] = (double)f.z; v[3] = (double)f.w;
+}
+__device__ __forceinline__ void st_b4(double* p, double a, double b, double c, double d) { st32(p, a, b, c, d); }
+__device__ __forceinline__ void st_b4(float* p, double a, double b, double c, double d)
+{
+  asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"((float)a), "f"((float)b), "f"((float)c), "f"((float)d) : "memory");
+}
+template <typename TB> __device__ __forceinline__ TB* carried_inverse(const CrowdDev& d);
+template <> __device__ __forceinline__ double* carried_inverse<double>(const CrowdDev& d) { return d.Binv; }
+template <> __device__ __forceinline__ float* carried_inverse<float>(const CrowdDev& d) { return d.Binv32; }
 
 // Flush, step 1 (per walker, column-local): Z = S^-T C, Z[l][j] = sum_q Sinv[q][l] C[q][j], written to
 // the d.C buffer, so that the strip kernel needs two GEMMs only: B <- B0 - (B0 V^T - E) Z.  C[q] is read
@@ -150,14 +202,14 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d,
   const int j = blockIdx.x * COLS + (threadIdx.x - half * COLS);
   const int l0 = half * ZL;
   double* C = d.C + (size_t)w * KDP * ns + j;
-  const double* B0 = d.Binv + ((size_t)w * 2 + spin) * ns * ns + j;
+  const size_t B0 = ((size_t)w * 2 + spin) * ns * ns + j;
   double z[ZL];
 #pragma unroll
   for (int l = 0; l < ZL; ++l) z[l] = 0.0;
   if (j < ns && l0 < m) {
 #pragma unroll 2
     for (int q = 0; q < m; ++q) {
-      const double c = B0[(size_t)s_rows[q] * ns];
+      const double c = ld_binv(d, B0 + (size_t)s_rows[q] * ns);
 #pragma unroll
       for (int l = 0; l < ZL; ++l) z[l] = fma(s_sinv[q * KDP + l0 + l], c, z[l]);
     }
@@ -273,12 +325,12 @@ template <int KB>
 struct Frag1 {
   double a0[4], a1[4], v[KB][4];
 };
-template <int KB>
-__device__ __forceinline__ void load_frag1(Frag1<KB>& f, const double* a0p, const double* a1p, const double* vp,
+template <int KB, typename TB>
+__device__ __forceinline__ void load_frag1(Frag1<KB>& f, const TB* a0p, const TB* a1p, const double* vp,
                                            int s, int ns, int m, int mb, int g)
 {
-  ld32(a0p + s, f.a0);
-  ld32(a1p + s, f.a1);
+  ld_b4(a0p + s, f.a0);
+  ld_b4(a1p + s, f.a1);
 #pragma unroll
   for (int b = 0; b < KB; ++b) {
     f.v[b][0] = f.v[b][1] = f.v[b][2] = f.v[b][3] = 0.0;
@@ -305,12 +357,12 @@ struct Frag2 {
   double x0[4], x1[4];
   double2 z[KB][2];
 };
-template <int KB>
-__device__ __forceinline__ void load_frag2(Frag2<KB>& f, const double* a0p, const double* a1p, const double* zp,
+template <int KB, typename TB>
+__device__ __forceinline__ void load_frag2(Frag2<KB>& f, const TB* a0p, const TB* a1p, const double* zp,
                                            int j0, int ns, int m, int mb, int t)
 {
-  ld32(a0p + j0, f.x0);
-  ld32(a1p + j0, f.x1);
+  ld_b4(a0p + j0, f.x0);
+  ld_b4(a1p + j0, f.x1);
 #pragma unroll
   for (int b = 0; b < KB; ++b)
 #pragma unroll
@@ -319,9 +371,9 @@ __device__ __forceinline__ void load_frag2(Frag2<KB>& f, const double* a0p, cons
       if (b < mb && 8 * b + 2 * t + q < m) f.z[b][q] = *reinterpret_cast<const double2*>(zp + (size_t)(8 * b + q) * ns + j0);
     }
 }
-template <int KB>
-__device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double (&nw)[2][KB][2], int mb, double* o0,
-                                                double* o1)
+template <int KB, typename TB>
+__device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double (&nw)[2][KB][2], int mb, TB* o0,
+                                                TB* o1)
 {
   // even / odd columns of the chunk are separate tiles (a lane ends up with 4 consecutive columns);
   // two accumulator sets (even / odd window blocks) give 8 independent DMMA chains, summed at the end
@@ -345,14 +397,16 @@ __device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double
           dmma884(do1, nw[1][b][q], f.z[b][q].y);
         }
       }
-  st32(o0, de0[0] + ee0[0], do0[0] + eo0[0], de0[1] + ee0[1], do0[1] + eo0[1]);
-  st32(o1, de1[0] + ee1[0], do1[0] + eo1[0], de1[1] + ee1[1], do1[1] + eo1[1]);
+  st_b4(o0, de0[0] + ee0[0], do0[0] + eo0[0], de0[1] + ee0[1], do0[1] + eo0[1]);
+  st_b4(o1, de1[0] + ee1[0], do1[0] + eo1[0], de1[1] + ee1[1], do1[1] + eo1[1]);
 }
 
 // Flush, step 2: B_strip <- B0_strip - (B0_strip V^T - E) Z.  KB = kdp / 8. grid = (ceil(ns / 64), W).
 // L0: first move of the section this launch applies (-1: the whole window; a compile-time constant, so the common
 // case keeps the register allocation it was tuned with)
-template <int KB, int L0 = -1>
+// TB: storage type of the carried inverse (double; float = mixed precision, D:R6: fragments widened on load, the
+// updated strip rounded to fp32 once on store -- 8 n^2 bytes per walker-flush instead of 16 n^2)
+template <int KB, int L0 = -1, typename TB = double>
 __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(CrowdDev d, int spin)
 {
   constexpr int l0 = L0 < 0 ? 0 : L0;
@@ -369,11 +423,11 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int row0 = (blockIdx.x * (FLUSH_NT / 32) + warp) * FLUSH_ROWS_PER_WARP;
   if (row0 >= ns) return;
-  double* B = d.Binv + ((size_t)w * 2 + spin) * ns * ns;
+  TB* B = carried_inverse<TB>(d) + ((size_t)w * 2 + spin) * ns * ns;
   const int* rows = d.rows + (size_t)w * kdp + l0;
   const int mb = (m + 7) >> 3;  // 8-wide blocks of the window that hold accepted moves
-  double* a0p = B + (size_t)(row0 + g) * ns + 4 * t;
-  double* a1p = a0p + (size_t)8 * ns;
+  TB* a0p = B + (size_t)(row0 + g) * ns + 4 * t;
+  TB* a1p = a0p + (size_t)8 * ns;
   // lane's V fragment base: row g of each window block, columns 4t..4t+3 of the chunk
   const double* vp = d.V + (size_t)w * kdp * ns + (size_t)(g + l0) * ns + 4 * t;
   // lane's Z fragment base: rows 2t (+q) of each window block, columns 2g, 2g+1 of the chunk

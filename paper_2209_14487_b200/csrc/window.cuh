@@ -23,6 +23,7 @@
 // factor (flush_finalize_tri_kernel); the two-GEMM strip kernel is the same for both paths.
 #pragma once
 #include "move.cuh"
+#include "update.cuh"
 
 namespace qmc {
 
@@ -208,8 +209,15 @@ __device__ __forceinline__ void cp_async_warp(void* smem, const void* gmem, int 
 // dot and the update (rows of up to 64 WIN_NV = 512 columns; longer rows are read twice), and also
 // hands row r_first to shared memory (next_s) as the next move's inverse row.
 constexpr int WIN_NV = 8;
-template <typename T, int NT>
-__device__ __forceinline__ void block_rows_update(const double* src, double* dst, int ns, int r_first, int cnt,
+// TS: type of the source rows (double; float when they are still the fp32-stored B0 rows of the mixed-precision mode)
+__device__ __forceinline__ double2 ld_row2(const double* row, int jj) { return reinterpret_cast<const double2*>(row)[jj]; }
+__device__ __forceinline__ double2 ld_row2(const float* row, int jj)
+{
+  const float2 f = reinterpret_cast<const float2*>(row)[jj];
+  return make_double2((double)f.x, (double)f.y);
+}
+template <typename T, int NT, typename TS = double>
+__device__ __forceinline__ void block_rows_update(const TS* src, double* dst, int ns, int r_first, int cnt,
                                                   const T* vgl_s, const double* c_s, double* next_s)
 {
   constexpr int RB = 2;
@@ -222,11 +230,11 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
 #pragma unroll
       for (int r = 0; r < RB; ++r) {
         acc[r] = 0.0;
-        const double2* rp = reinterpret_cast<const double2*>(src + (size_t)(r0 + r) * ns);
+        const TS* rp = src + (size_t)(r0 + r) * ns;
 #pragma unroll
         for (int q = 0; q < WIN_NV; ++q) {
           const int jj = lane + 32 * q;
-          v[r][q] = (r0 + r < cnt && jj < nh) ? rp[jj] : make_double2(0.0, 0.0);
+          v[r][q] = (r0 + r < cnt && jj < nh) ? ld_row2(rp, jj) : make_double2(0.0, 0.0);
         }
       }
 #pragma unroll
@@ -260,16 +268,16 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
     }
   } else {
     for (int r = r_first + warp; r < cnt; r += NT / 32) {
-      const double2* rp = reinterpret_cast<const double2*>(src + (size_t)r * ns);
+      const TS* rp = src + (size_t)r * ns;
       double2* wp = reinterpret_cast<double2*>(dst + (size_t)r * ns);
       double acc = 0.0;
       for (int jj = lane; jj < nh; jj += 32) {
-        const double2 x = ld_x2(vgl_s, jj), v = rp[jj];
+        const double2 x = ld_x2(vgl_s, jj), v = ld_row2(rp, jj);
         acc = fma(v.x, x.x, fma(v.y, x.y, acc));
       }
       acc = warp_sum(acc);
       for (int jj = lane; jj < nh; jj += 32) {
-        const double2 c = c2[jj], v = rp[jj];
+        const double2 c = c2[jj], v = ld_row2(rp, jj);
         const double2 o = make_double2(fma(-acc, c.x, v.x), fma(-acc, c.y, v.y));
         wp[jj] = o;
         if (r == r_first) reinterpret_cast<double2*>(next_s)[jj] = o;
@@ -288,7 +296,9 @@ __device__ __forceinline__ void block_rows_update(const double* src, double* dst
 // NS > 0: the kernel is specialised for n = M = ns = NS (N = 2 NS, a table stride that covers ns): every trip count
 // and row stride is a compile-time constant, loops unroll and the index arithmetic folds -- the kernel is bound by its
 // instruction stream, a third of which was integer / control overhead (ncu r2).  NS = 0: any shape.
-template <typename T, int NT, int NS = 0>
+// TB: storage type of the carried inverse (double; float = mixed precision, D:R6: the block's B0 rows are widened
+// on load; everything the window itself writes -- Bcur, V, Cp -- stays fp64).
+template <typename T, int NT, int NS = 0, typename TB = double>
 __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) window_kernel(CrowdDev d, int k0, int cnt)
 {
   extern __shared__ double sm[];
@@ -308,7 +318,8 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
   const MoveScal ms = move_scal_smem(sm + L.mv);
 
   const int spin = k0 / sh_n<NS>(d), kk0 = k0 - spin * sh_n<NS>(d);
-  const double* blk = d.Binv + (((size_t)w * 2 + spin) * ns + kk0) * ns;  // B0 rows of the window
+  const TB* blk = carried_inverse<TB>(d) + (((size_t)w * 2 + spin) * ns + kk0) * ns;  // B0 rows of the window
+  constexpr bool B64 = sizeof(TB) == 8;
   double* Bcur = d.C + (size_t)w * kdp * ns;                              // their current values, once m > 0
   double* Cp = d.Cp + (size_t)w * kdp * ns;
   double* V = d.V + (size_t)w * kdp * ns;
@@ -318,11 +329,13 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
 
   // prologue: row and gradient cache of the first move, positions, Gaussians of the first move;
   // the rest of the block is pulled into L2 (first-touch DRAM lines the first accepted move reads)
-  cp_async_cta<NT>(b_s, blk, row_bytes);
+  if constexpr (B64) cp_async_cta<NT>(b_s, blk, row_bytes);
+  else
+    for (int j = tid; j < ns; j += NT) b_s[j] = (double)blk[j];
   cp_async_cta<NT>(cbuf, cache0, cache_bytes);
   for (int j = tid; j < 3 * nN; j += NT) R_s[j] = Rg[j];
   if (tid >= 32 && tid < 37) gauss[tid - 32] = gauss_piece(d, w, k0, tid - 32);
-  for (int j = tid; j < (cnt - 1) * row_bytes / 128; j += NT)
+  for (int j = tid; j < (cnt - 1) * ns * (int)sizeof(TB) / 128; j += NT)
     asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
   cp_async_wait_all();
   __syncthreads();
@@ -386,7 +399,9 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
         }
       }
       if (warp == 3 % (NT / 32)) {
-        cp_async_warp(bn_s, (m ? Bcur : blk) + (size_t)(i + 1) * ns, row_bytes);
+        if (B64 || m) cp_async_warp(bn_s, (m ? Bcur : reinterpret_cast<const double*>(blk)) + (size_t)(i + 1) * ns, row_bytes);
+        else
+          for (int j = lane; j < ns; j += 32) bn_s[j] = (double)blk[(size_t)(i + 1) * ns + j];
         cp_async_warp(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
       }
     }
@@ -410,7 +425,9 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
       if (tid == 0) rows_s[m] = kk0 + i;
       cp_async_wait_all();   // the stale copy of the next row has landed before the update overwrites it
       __syncthreads();
-      block_rows_update<T, NT>(m ? Bcur : blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
+      if constexpr (B64) block_rows_update<T, NT>(m ? Bcur : reinterpret_cast<const double*>(blk), Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
+      else if (m) block_rows_update<T, NT>(Bcur, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
+      else block_rows_update<T, NT, TB>(blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
       ++m;
     }
     cp_async_wait_all();
