@@ -222,84 +222,6 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d,
   }
 }
 
-// Flush, step 1 for the window kernel's eager-block form (window.cuh, DESIGN.md R5): the accepted moves
-// left V[l] = phi_l and Cp[l] = c_l = b_l / rho_l; with N[j][l] = c_j . phi_l (j < l, strictly upper
-// triangular) the Sherman-Morrison chain B_m = B0 - sum_l w_l c_l^T, w_l = B_l phi_l - e_l, telescopes to
-// B_m = B0 - (B0 V^T - E) Z with (I + N) Z = Cp.  One CTA per walker: N by DMMA tiles (operand
-// fragments straight from the rows of Cp and V, as in the strip kernel), then back substitution, one
-// column per thread, Z written to the d.C buffer.  m^2 n + m^2 n / 2 flop per walker (5 % of the flush).
-// grid = W; dynamic smem: KDP*(KDP+1) doubles
-#ifndef QMC_FINTRI_MIN_CTAS
-#define QMC_FINTRI_MIN_CTAS 4
-#endif
-constexpr int FINTRI_NT = 128;
-template <int KDP>
-__global__ void __launch_bounds__(FINTRI_NT, KDP > 32 ? 2 : QMC_FINTRI_MIN_CTAS) flush_finalize_tri_kernel(CrowdDev d, int l0)
-{
-  // l0 > 0: the window is flushed in sections of KDP accepted moves (section = moves l0 .. l0 + KDP - 1), each section a
-  // complete flush of its own applied to the result of the previous one (see launch_flush_kdp)
-  constexpr int KB = KDP / 8, SS = KDP + 1;
-  extern __shared__ double s_n[];
-  const int w = blockIdx.x + d.w0;
-  const int m = min(d.mwin[w] - l0, KDP);
-  if (m <= 0) return;
-  const int ns = d.ns, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-  const double* Cp = d.Cp + ((size_t)w * d.kdp + l0) * ns;
-  const double* V = d.V + ((size_t)w * d.kdp + l0) * ns;
-  double* Z = d.C + ((size_t)w * d.kdp + l0) * ns;
-  for (int e = tid; e < KDP * SS; e += FINTRI_NT) s_n[e] = 0.0;
-  __syncthreads();
-  for (int jb = warp; jb < KB && 8 * jb < m; jb += FINTRI_NT / 32) {
-    double acc[KB][2];
-#pragma unroll
-    for (int lb = 0; lb < KB; ++lb) acc[lb][0] = acc[lb][1] = 0.0;
-    const bool a_ok = 8 * jb + g < m;
-    const double* ap = Cp + (size_t)(8 * jb + g) * ns + 4 * t;
-    const double* vp = V + (size_t)g * ns + 4 * t;
-#pragma unroll 2   // two chunks of fragment loads in flight (the loop is a chain of L2 round trips otherwise)
-    for (int s = 0; s < ns; s += 16) {
-      double a[4] = {0.0, 0.0, 0.0, 0.0};
-      if (a_ok) ld32(ap + s, a);
-      double b[KB][4];
-#pragma unroll
-      for (int lb = 0; lb < KB; ++lb) {
-        b[lb][0] = b[lb][1] = b[lb][2] = b[lb][3] = 0.0;
-        if (lb >= jb && 8 * lb + g < m) ld32(vp + (size_t)(8 * lb) * ns + s, b[lb]);
-      }
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-#pragma unroll
-        for (int lb = 0; lb < KB; ++lb)
-          if (lb >= jb) dmma884(acc[lb], a[q], b[lb][q]);
-    }
-#pragma unroll
-    for (int lb = 0; lb < KB; ++lb)
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int j = 8 * jb + g, l = 8 * lb + 2 * t + e;
-        if (lb >= jb && j < l && l < m) s_n[j * SS + l] = acc[lb][e];
-      }
-  }
-  __syncthreads();
-  for (int col = tid; col < ns; col += FINTRI_NT) {
-    double z[KDP];
-#pragma unroll
-    for (int l = 0; l < KDP; ++l) z[l] = (l < m) ? Cp[(size_t)l * ns + col] : 0.0;
-#pragma unroll
-    for (int l = KDP - 2; l >= 0; --l) {
-      if (l < m - 1) {
-        double a = z[l];
-#pragma unroll
-        for (int j = l + 1; j < KDP; ++j) a = fma(-s_n[l * SS + j], z[j], a);
-        z[l] = a;
-      }
-    }
-#pragma unroll
-    for (int l = 0; l < KDP; ++l)
-      if (l < m) Z[(size_t)l * ns + col] = z[l];
-  }
-}
-
 // Measured alternatives on B200 (cfg 5, W = 4096, round 1):
 //  - the DMMA.8x8x4 issue ceiling with this chain structure is 37.2 TFLOP/s, and 34.4 TFLOP/s with the V and strip
 //    fragments loaded straight from L1/L2 as here -- the operand path is not the limit, DRAM streaming is: the strip is
@@ -399,6 +321,120 @@ __device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double
       }
   st_b4(o0, de0[0] + ee0[0], do0[0] + eo0[0], de0[1] + ee0[1], do0[1] + eo0[1]);
   st_b4(o1, de1[0] + ee1[0], do1[0] + eo1[0], de1[1] + ee1[1], do1[1] + eo1[1]);
+}
+
+// Flush, step 1 for the window kernel's eager-block form (window.cuh, DESIGN.md R5): the accepted moves
+// left V[l] = phi_l and Cp[l] = c_l = b_l / rho_l; with N[j][l] = c_j . phi_l (j < l, strictly upper
+// triangular) the Sherman-Morrison chain B_m = B0 - sum_l w_l c_l^T, w_l = B_l phi_l - e_l, telescopes to
+// B_m = B0 - (B0 V^T - E) Z with (I + N) Z = Cp.  One CTA per walker, three steps, all on the FP64 tensor pipe but
+// the tiny middle one:
+//   1. N by DMMA tiles (operand fragments straight from the rows of Cp and V, as in the strip kernel);
+//   2. T = (I + N)^-1, unit upper triangular, by back substitution on the identity: one warp, lane = column, the
+//      column in registers (496 fused multiply-adds per lane);
+//   3. Z = T Cp by DMMA tiles in the strip kernel's GEMM-2 fragment scheme (T from shared memory as the A operand,
+//      rows of Cp as the B operand, four consecutive columns of Z per lane and store).
+// (Round 1 solved (I + N) Z = Cp by back substitution with one column of Z per thread: 32 dependent values in
+// registers next to the DMMA code spilled 440 bytes per thread under the 128-register cap.)
+// m^2 n + 2 m^2 n flop per walker.  grid = W; dynamic smem: 2 KDP (KDP + 1) doubles.
+#ifndef QMC_FINTRI_MIN_CTAS
+#define QMC_FINTRI_MIN_CTAS 3
+#endif
+constexpr int FINTRI_NT = 128;
+template <int KDP>
+__global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize_tri_kernel(CrowdDev d, int l0)
+{
+  // l0 > 0: the window is flushed in sections of KDP accepted moves (section = moves l0 .. l0 + KDP - 1), each section a
+  // complete flush of its own applied to the result of the previous one (see launch_flush_kdp)
+  static_assert(KDP % 16 == 0 || KDP == 8, "two 8-row blocks per output strip");
+  constexpr int KB = KDP / 8, SS = KDP + 1;
+  extern __shared__ double s_n[];
+  double* s_t = s_n + KDP * SS;
+  const int w = blockIdx.x + d.w0;
+  const int m = min(d.mwin[w] - l0, KDP);
+  if (m <= 0) return;
+  const int ns = d.ns, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+  const double* Cp = d.Cp + ((size_t)w * d.kdp + l0) * ns;
+  const double* V = d.V + ((size_t)w * d.kdp + l0) * ns;
+  double* Z = d.C + ((size_t)w * d.kdp + l0) * ns;
+  for (int e = tid; e < KDP * SS; e += FINTRI_NT) s_n[e] = 0.0;
+  __syncthreads();
+  // ---- 1. N[j][l] = Cp[j] . V[l] for j < l < m
+  for (int jb = warp; jb < KB && 8 * jb < m; jb += FINTRI_NT / 32) {
+    double acc[KB][2];
+#pragma unroll
+    for (int lb = 0; lb < KB; ++lb) acc[lb][0] = acc[lb][1] = 0.0;
+    const bool a_ok = 8 * jb + g < m;
+    const double* ap = Cp + (size_t)(8 * jb + g) * ns + 4 * t;
+    const double* vp = V + (size_t)g * ns + 4 * t;
+#pragma unroll 2   // two chunks of fragment loads in flight (the loop is a chain of L2 round trips otherwise)
+    for (int s = 0; s < ns; s += 16) {
+      double a[4] = {0.0, 0.0, 0.0, 0.0};
+      if (a_ok) ld32(ap + s, a);
+      double b[KB][4];
+#pragma unroll
+      for (int lb = 0; lb < KB; ++lb) {
+        b[lb][0] = b[lb][1] = b[lb][2] = b[lb][3] = 0.0;
+        if (lb >= jb && 8 * lb + g < m) ld32(vp + (size_t)(8 * lb) * ns + s, b[lb]);
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+#pragma unroll
+        for (int lb = 0; lb < KB; ++lb)
+          if (lb >= jb) dmma884(acc[lb], a[q], b[lb][q]);
+    }
+#pragma unroll
+    for (int lb = 0; lb < KB; ++lb)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int j = 8 * jb + g, l = 8 * lb + 2 * t + e;
+        if (lb >= jb && j < l && l < m) s_n[j * SS + l] = acc[lb][e];
+      }
+  }
+  __syncthreads();
+  // ---- 2. T = (I + N)^-1: column c solves (I + N) x = e_c from the bottom up; x[l] = 0 below the diagonal
+  if (warp == 0 && lane < KDP) {
+    const int c = lane;
+    double x[KDP];
+#pragma unroll
+    for (int l = KDP - 1; l >= 0; --l) {
+      double a = 0.0;
+#pragma unroll
+      for (int j = l + 1; j < KDP; ++j) a = fma(-s_n[l * SS + j], x[j], a);
+      x[l] = l < c ? a : (l == c ? 1.0 : 0.0);
+    }
+#pragma unroll
+    for (int l = 0; l < KDP; ++l) s_t[l * SS + c] = x[l];
+  }
+  __syncthreads();
+  // ---- 3. Z = T Cp: a warp takes the 16-row strips of Z and 16-column chunks in turn
+  constexpr int NSTRIP = KDP >= 16 ? KDP / 16 : 1, RB = KDP >= 16 ? 2 : 1;
+  const int mb = (m + 7) >> 3;
+  for (int item = warp; item < NSTRIP * (ns / 16); item += FINTRI_NT / 32) {
+    const int strip = item % NSTRIP, j0 = (item / NSTRIP) * 16;
+    if (16 * strip >= m) continue;
+    // T as the A operand of the strip kernel's GEMM 2: rows 16 strip + 8 i + g, contraction index 8 b + 2 t + e
+    double nw[2][KB][2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int b = 0; b < KB; ++b)
+#pragma unroll
+        for (int e = 0; e < 2; ++e)
+          nw[i][b][e] = s_t[(16 * strip + 8 * (i % RB) + g) * SS + 8 * b + 2 * t + e];
+    Frag2<KB> f;
+    f.x0[0] = f.x0[1] = f.x0[2] = f.x0[3] = 0.0;
+    f.x1[0] = f.x1[1] = f.x1[2] = f.x1[3] = 0.0;
+#pragma unroll
+    for (int b = 0; b < KB; ++b)
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        f.z[b][q] = make_double2(0.0, 0.0);
+        if (b < mb && 8 * b + 2 * t + q < m) f.z[b][q] = *reinterpret_cast<const double2*>(Cp + (size_t)(8 * b + 2 * t + q) * ns + j0 + 2 * g);
+      }
+    double* o0 = Z + (size_t)(16 * strip + g) * ns + 4 * t + j0;
+    // KDP = 8 has one row block: the second one repeats it (same values to the same addresses)
+    mma_store_frag2<KB>(f, nw, mb, o0, RB == 2 ? o0 + (size_t)8 * ns : o0);
+  }
 }
 
 // Flush, step 2: B_strip <- B0_strip - (B0_strip V^T - E) Z.  KB = kdp / 8. grid = (ceil(ns / 64), W).
