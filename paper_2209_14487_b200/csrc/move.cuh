@@ -142,20 +142,25 @@ __device__ __forceinline__ void sinv_matvec(const double* Sinv, int ss, int m, c
   }
 }
 
-// Piece 0..4 of the Box-Muller Gaussians of move (walker w, electron k, current sweep) (D:C7):
+// The five Box-Muller pieces of the Gaussians of move (walker w, electron k, current sweep) (D:C7):
 // chi = (g0 g1, g0 g2, g3 g4), g0 = sqrt(-2 ln u0), g1 = cos 2 pi u1, g2 = sin 2 pi u1, g3 = sqrt(-2 ln u2),
-// g4 = cos 2 pi u3.  One thread per piece; the pieces depend on nothing but the counter, so the window
-// kernel computes them ahead of time, off the critical path.
-__device__ __forceinline__ double gauss_piece(const CrowdDev& d, int w, int k, int piece)
+// g4 = cos 2 pi u3.  Four lanes (part = 0..3) of one warp: parts 0 / 2 take the two radii, parts 1 / 3 the two angles
+// (sincos: one argument reduction for g1 and g2), so the warp runs two code paths instead of five.  The pieces depend
+// on nothing but the counter, so the window kernel computes them ahead of time, off the critical path.
+// out[0..4] = g0..g4; callers synchronise before reading.
+__device__ __forceinline__ void gauss_pieces(const CrowdDev& d, int w, int k, int part, double* out)
 {
   unsigned x[4];
   philox4x32_10((unsigned)(d.walker_id0 + w), (unsigned)k, *d.sweep, 0u, d.seed_lo, d.seed_hi, x);
   const double two_pi = 6.283185307179586476925286766559;
-  if (piece == 0) return sqrt(-2.0 * log(u01(x[0])));
-  if (piece == 1) return cos(two_pi * u01(x[1]));
-  if (piece == 2) return sin(two_pi * u01(x[1]));
-  if (piece == 3) return sqrt(-2.0 * log(u01(x[2])));
-  return cos(two_pi * u01(x[3]));
+  if ((part & 1) == 0) {
+    out[part == 0 ? 0 : 3] = sqrt(-2.0 * log(u01(x[part])));
+  } else {
+    double sn, cs;
+    sincos(two_pi * u01(x[part]), &sn, &cs);
+    if (part == 1) { out[1] = cs; out[2] = sn; }
+    else out[4] = cs;
+  }
 }
 
 // ---- G_k(R) and the proposal (qmc_spo_vgl step (b)) -------------------------------------------
@@ -187,7 +192,7 @@ __device__ __forceinline__ void dev_gold_propose(const CrowdDev& d, int w, int k
   }
   block_sum_t0<7, NT>(v, red);
   if (!rnew_given && !gauss_pre) {
-    if (tid < 5) red[tid] = gauss_piece(d, w, k, tid);
+    if (tid < 4) gauss_pieces(d, w, k, tid, red);
     __syncthreads();
   }
   const double* gp = gauss_pre ? gauss_pre : red;

@@ -208,7 +208,9 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
   for (unsigned c0 = 0; c0 < chunks; c0 += NT / 4) {
     const unsigned chunk = c0 + g;
     T out[5][VW];
-    if (chunk < sh_tab_vecs<NS>(d) && chunk < chunks) {
+    // shape known at compile time with the slices filling every round: no bounds checks, no masking of padding columns
+    constexpr bool FULL = NS > 0 && (NS / VW) % (NT / 4) == 0;
+    if (FULL || (chunk < sh_tab_vecs<NS>(d) && chunk < chunks)) {
       T p[4][4][VW];
       spline_plane_load<T, KEEP>(tab, s, a, chunk, p);
       if (c0 == 0 && tid >= 32) side(tid);
@@ -243,8 +245,8 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
     }
 #pragma unroll
     for (int e = 0; e < VW; ++e)
-      if ((int)(chunk * VW) + e >= sh_M<NS>(d)) f0[e] = f1[e] = (T)0;
-    if (chunk < chunks) {
+      if (!FULL && (int)(chunk * VW) + e >= sh_M<NS>(d)) f0[e] = f1[e] = (T)0;
+    if (FULL || chunk < chunks) {
       T* o = vgl + (size_t)chunk * VW;
       st16(o + (size_t)a * sh_ns<NS>(d), f0);
       if (a == 0) st16(o + (size_t)4 * sh_ns<NS>(d), f1);

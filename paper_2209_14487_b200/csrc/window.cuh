@@ -334,7 +334,7 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
     for (int j = tid; j < ns; j += NT) b_s[j] = (double)blk[j];
   cp_async_cta<NT>(cbuf, cache0, cache_bytes);
   for (int j = tid; j < 3 * nN; j += NT) R_s[j] = Rg[j];
-  if (tid >= 32 && tid < 37) gauss[tid - 32] = gauss_piece(d, w, k0, tid - 32);
+  if (tid >= 32 && tid < 36) gauss_pieces(d, w, k0, tid - 32, gauss);
   for (int j = tid; j < (cnt - 1) * ns * (int)sizeof(TB) / 128; j += NT)
     asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
   cp_async_wait_all();
@@ -386,7 +386,7 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
     if (more) {
       const int warp = tid >> 5, lane = tid & 31;
       if (warp == 1 % (NT / 32)) {
-        if (lane < 5) gauss[lane] = gauss_piece(d, w, k + 1, lane);
+        if (lane < 4) gauss_pieces(d, w, k + 1, lane, gauss);
       }
       if (warp == 2 % (NT / 32)) {
         if (lane >= 30) {
@@ -416,7 +416,8 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
         Cp[(size_t)m * ns + j] = c;
         V[(size_t)m * ns + j] = (double)vgl_s[j];
       }
-      for (int j = tid; j < 4 * ns; j += NT) cache_g[j] = vgl_s[ns + j];
+      for (int j = tid; j < 4 * ns * (int)sizeof(T) / 16; j += NT)   // gradient / Laplacian cache of electron k, 16 bytes at a time
+        reinterpret_cast<float4*>(cache_g)[j] = reinterpret_cast<const float4*>(vgl_s + ns)[j];
       if (tid < 3) {
         const double x = ms.rn[tid];
         R_s[3 * k + tid] = x;
@@ -528,7 +529,7 @@ __global__ void __launch_bounds__(MOVE_NT, 512 / MOVE_NT) sweep1_kernel(CrowdDev
   cp_async_cta(b_s, Bw, row_bytes);
   cp_async_cta(cbuf, cache0, cache_bytes);
   for (int j = tid; j < 3 * d.N; j += MOVE_NT) R_s[j] = Rg[j];
-  if (tid >= 32 && tid < 37) gauss[tid - 32] = gauss_piece(d, w, 0, tid - 32);
+  if (tid >= 32 && tid < 36) gauss_pieces(d, w, 0, tid - 32, gauss);
   cp_async_wait_all();
   __syncthreads();
 
@@ -545,7 +546,7 @@ __global__ void __launch_bounds__(MOVE_NT, 512 / MOVE_NT) sweep1_kernel(CrowdDev
     }
     dev_gold_propose<T>(d, w, k, b_s, ccur, R_s, nullptr, ms, red, gauss, &sw);
     spline_cta<T, MOVE_NT>(d, nullptr, sw, vgl_s, [&](int t) {
-      if (more && t < 37) gauss[t - 32] = gauss_piece(d, w, k + 1, t - 32);
+      if (more && t < 36) gauss_pieces(d, w, k + 1, t - 32, gauss);
     });
     __syncthreads();
     dev_ratio_grad<T>(d, w, k, b_s, vgl_s, R_s, ms, nullptr, nullptr, red);
