@@ -224,26 +224,24 @@ __device__ __forceinline__ void warp_sum8(double (&v)[8])
   for (int q = 0; q < 8; ++q) v[q] = __shfl_sync(0xffffffffu, e, ((q >> 2) & 1) * 16 + ((q >> 1) & 1) * 8 + (q & 1) * 4);
 }
 
-// 1/x and 1/sqrt(x) for normal positive x: the hardware's approximate seed (MUFU.RCP64H / RSQ64H, ~2^-23) and two Newton
-// steps in fma arithmetic (~2^-46, then full double precision to within an ulp or two), without the special-case
-// branches of the library versions.  Used by the Jastrow pair terms, whose arguments are well inside the normal range.
+// 1/x and 1/sqrt(x) for normal positive x: the hardware's approximate seed (MUFU.RCP64H / RSQ64H, relative error e with
+// |e| < 2^-22) and ONE third-order correction in fma arithmetic -- 1/x = y (1 + e + e^2 + O(e^3)) with e = 1 - x y,
+// 1/sqrt(x) = y (1 + e/2 + 3 e^2/8 + O(e^3)) with e = 1 - x y^2 -- i.e. full double precision to within an ulp or two
+// (the neglected terms are below 2^-66), without the special-case branches of the library versions.  Used by the
+// Jastrow pair terms, whose arguments are well inside the normal range.
 __device__ __forceinline__ double rcp_pos(double x)
 {
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = fma(-x, y, 1.0);
-  y = fma(y, e, y);
-  e = fma(-x, y, 1.0);
-  return fma(y, e, y);
+  const double e = fma(-x, y, 1.0);
+  return fma(y, fma(e, e, e), y);
 }
 __device__ __forceinline__ double rsqrt_pos(double x)
 {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = fma(-(x * y), 0.5 * y, 0.5);
-  y = fma(y, e, y);
-  e = fma(-(x * y), 0.5 * y, 0.5);
-  return fma(y, e, y);
+  const double e = fma(-(x * y), y, 1.0);
+  return fma(y, e * fma(e, 0.375, 0.5), y);
 }
 
 // ---- Philox4x32-10 (Salmon et al., SC'11; D:C7). Counter (walker id, k, sweep, tag). ----
