@@ -237,6 +237,20 @@ __global__ void __launch_bounds__(FINALIZE_NT) flush_finalize_kernel(CrowdDev d,
 //  - a pair of warps per strip splitting its columns (partials exchanged through shared memory, second read half a
 //    strip after the first): 4.4 ms instead of 3.5 ms -- the exposed load latency at the start of each shorter
 //    GEMM loop costs more than the L2 hits save.
+// Round 2 (measured on B200 at cfg 5, W = 4096):
+//  - the strip staged ONCE in shared memory by bulk asynchronous copies (cp.async.bulk + mbarrier, one copy per row issued
+//    by a lane, rows padded by 16 bytes so that the fragment reads are conflict-free; persistent grid, one CTA per SM;
+//    both GEMMs take the strip from shared memory, V / Z fragments software-pipelined 4 chunks ahead in registers at 255
+//    registers per thread): correct (same tests), DRAM traffic at the algorithmic minimum, and SLOWER -- 8-row strips,
+//    4 warps per SM, strip double-buffered (198 KB): 7.1 ms per flush; 8 warps per SM, single-buffered: 5.1 ms; against
+//    3.1 ms for this kernel.  With ~200 KB of shared memory the L1 shrinks to ~30 KB, the V and Z fragments (196 KB per
+//    walker, read once per strip) come from L2 every time, and 4-8 warps per SM cannot hide that latency next to the
+//    DMMAs; 16-row strips need 48 KB per warp, which leaves room for neither a second buffer nor a fifth warp.  The
+//    variant was removed again;
+//  - storing the inverses in fp32 (mixed precision, half the strip bytes) leaves the time of this kernel unchanged, a fourth
+//    CTA per SM at 128 registers spills 472 bytes, ns as a compile-time constant changes nothing: the kernel is bound by
+//    the latency of its fragment loads at 12 warps per SM (65 % of its stall samples are the first DMMA of a fragment set
+//    waiting for that set), not by DRAM bandwidth and not by instruction issue.
 // ---- strip kernel: fragments straight from global memory, software-pipelined in registers -------
 // (A shared-memory cp.async ring for the operands was measured slower on B200 in round 1: 2.54 ms vs 2.07 ms per
 // flush at cfg 5 / W = 2048 -- the LDS + LDGSTS instruction stream saturates the MIO queue next to
