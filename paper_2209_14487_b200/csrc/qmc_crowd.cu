@@ -445,7 +445,8 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   const int nt = window_threads(d.W);
   const size_t smem = window_smem(d, sizeof(T), nt);
   // shape-specialised instances for the BASELINE.json shapes with n a multiple of 16 (cfgs 3, 4, 5): see window.cuh
-  const bool spec = nt == 128 && sizeof(T) == 4 && d.n == d.ns && d.M == d.n && d.tab_vecs >= (unsigned)d.ns / 4;
+  const bool shape_ok = sizeof(T) == 4 && d.n == d.ns && d.M == d.n && d.tab_vecs >= (unsigned)d.ns / 4;
+  const bool spec = nt == 128 && shape_ok;
   if (d.Binv32) {   // mixed precision (D:R6): the block's B0 rows are fp32
     if (spec && d.ns == 384) window_kernel<T, 128, 384, float><<<wn, 128, smem, st>>>(d, k0, cnt);
     else if (nt == 512) window_kernel<T, 512, 0, float><<<wn, 512, smem, st>>>(d, k0, cnt);
@@ -454,6 +455,8 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   } else if (spec && d.ns == 384) window_kernel<T, 128, 384><<<wn, 128, smem, st>>>(d, k0, cnt);
   else if (spec && d.ns == 192) window_kernel<T, 128, 192><<<wn, 128, smem, st>>>(d, k0, cnt);
   else if (spec && d.ns == 96) window_kernel<T, 128, 96><<<wn, 128, smem, st>>>(d, k0, cnt);
+  else if (shape_ok && d.ns == 384 && nt == 256) window_kernel<T, 256, 384><<<wn, 256, smem, st>>>(d, k0, cnt);   // small crowds of cfg 5
+  else if (shape_ok && d.ns == 384 && nt == 512) window_kernel<T, 512, 384><<<wn, 512, smem, st>>>(d, k0, cnt);
   else switch (nt) {   // the class of the WHOLE crowd: a split into sub-crowds never changes a reduction tree
     case 512: window_kernel<T, 512><<<wn, 512, smem, st>>>(d, k0, cnt); break;
     case 256: window_kernel<T, 256><<<wn, 256, smem, st>>>(d, k0, cnt); break;
@@ -480,7 +483,8 @@ cudaError_t raise_smem_limits_t(int optin)
   const void* fns[] = {(const void*)row_propose_kernel<T>, (const void*)ratio_grad_kernel<T>, (const void*)accept_kernel<T>,
                        (const void*)ratio_accept_kernel<T>, (const void*)window_kernel<T, 128>,
                        (const void*)window_kernel<T, 128, 384>, (const void*)window_kernel<T, 128, 192>,
-                       (const void*)window_kernel<T, 128, 96>, (const void*)window_kernel<T, 128, 384, float>,
+                       (const void*)window_kernel<T, 128, 96>, (const void*)window_kernel<T, 256, 384>,
+                       (const void*)window_kernel<T, 512, 384>, (const void*)window_kernel<T, 128, 384, float>,
                        (const void*)window_kernel<T, 128, 0, float>, (const void*)window_kernel<T, 256, 0, float>,
                        (const void*)window_kernel<T, 512, 0, float>,
                        (const void*)window_kernel<T, 256>, (const void*)window_kernel<T, 512>,
