@@ -128,3 +128,19 @@ def test_anisotropic_grid_and_box(kd):
     for w in range(W):
         p, dp, d2p = osys.spo_vgl(mv[w])
         assert relerr(phi[w], p) < 1e-12 and relerr(dphi[w], dp) < 1e-12 and relerr(d2phi[w], d2p) < 1e-12
+
+
+def test_crowd_size_limit_is_checked_at_create():
+    """Several kernels put W (or 2 W) in gridDim.y (<= 65535): a crowd larger than 32767 walkers is refused with a clear
+    message instead of failing at a launch; a population that large is split into crowds."""
+    import torch
+    import paper_2209_14487_b200 as q
+    wl = qi.small_workload(n_elec=8, grid=4, box=3.0, coef_dtype="f32", coef_dist="normal", n_walkers=4, cfg=75)
+    coefs = torch.from_numpy(qi.make_coefs(wl)).cuda()
+    pos = torch.rand((32768, 8, 3), dtype=torch.float64, device="cuda") * 3.0
+    with pytest.raises(q.QmcError) as e:
+        q.Crowd(coefs, wl.box, pos, tau=0.01)
+    assert e.value.status == q.QMC_ERR_INVALID_ARG and "32767" in str(e.value)
+    c = q.Crowd(coefs, wl.box, pos[:32767].contiguous(), tau=0.01)
+    c.qmc_sweep(1)
+    assert c.stats()["proposed"] == 32767 * 8
