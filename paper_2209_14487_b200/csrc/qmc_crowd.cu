@@ -360,14 +360,14 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     // row over rho_l, whatever came before), and a section's Z solves only its own triangular block.  The strip kernel
     // with four window blocks keeps its double-buffered operands in registers (eight spill or lose the double
     // buffer): 11.1 -> 7.7 ms per flush of 64 moves at cfg 5, W = 4096.
-    flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)2 * 32 * 33 * 8, st>>>(d, 0);
+    flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)(1 + FINTRI_NT / 32) * 32 * 33 * 8, st>>>(d, 0);
     flush_kernel<4, 0><<<grid, FLUSH_NT, 0, st>>>(d, spin);
-    flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)2 * 32 * 33 * 8, st>>>(d, 32);
+    flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)(1 + FINTRI_NT / 32) * 32 * 33 * 8, st>>>(d, 32);
     flush_kernel<4, 32><<<grid, FLUSH_NT, 0, st>>>(d, spin);
     return;
   }
   if (from_window) {
-    if constexpr (KDP <= 32) flush_finalize_tri_kernel<KDP><<<wn, FINTRI_NT, (size_t)2 * KDP * (KDP + 1) * 8, st>>>(d, 0);
+    if constexpr (KDP <= 32) flush_finalize_tri_kernel<KDP><<<wn, FINTRI_NT, (size_t)(1 + FINTRI_NT / 32) * KDP * (KDP + 1) * 8, st>>>(d, 0);
   } else {
     const int fcols = FINALIZE_NT / (KDP > 32 ? KDP / 32 : 1);
     dim3 fgrid((d.ns + fcols - 1) / fcols, wn);

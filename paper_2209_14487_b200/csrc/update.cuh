@@ -349,7 +349,7 @@ __device__ __forceinline__ void mma_store_frag2(const Frag2<KB>& f, const double
 //      rows of Cp as the B operand, four consecutive columns of Z per lane and store).
 // (Round 1 solved (I + N) Z = Cp by back substitution with one column of Z per thread: 32 dependent values in
 // registers next to the DMMA code spilled 440 bytes per thread under the 128-register cap.)
-// m^2 n + 2 m^2 n flop per walker.  grid = W; dynamic smem: 2 KDP (KDP + 1) doubles.
+// m^2 n + 2 m^2 n flop per walker.  grid = W; dynamic smem: (1 + FINTRI_NT / 32) KDP (KDP + 1) doubles.
 #ifndef QMC_FINTRI_MIN_CTAS
 #define QMC_FINTRI_MIN_CTAS 3
 #endif
@@ -370,39 +370,61 @@ __global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize
   const double* Cp = d.Cp + ((size_t)w * d.kdp + l0) * ns;
   const double* V = d.V + ((size_t)w * d.kdp + l0) * ns;
   double* Z = d.C + ((size_t)w * d.kdp + l0) * ns;
+  // ---- 1. N[j][l] = Cp[j] . V[l] for j < l < m.  The contraction (over the ns columns) is split over the warps: a warp
+  // takes every fourth 16-column chunk and all (jb <= lb) tiles, so that each warp's chain of fragment loads is ns / 64
+  // chunks long instead of ns / 16, and the warps' work is equal (by rows of tiles, warp 0 had four tiles and warp 3
+  // one); the partial tiles meet in shared memory and are summed in a fixed order.
+  constexpr int NWF = FINTRI_NT / 32;
+  double* s_p = s_t + KDP * SS;   // [NWF - 1][KDP][SS] partial tiles of warps 1.. (warp 0 writes s_n)
   for (int e = tid; e < KDP * SS; e += FINTRI_NT) s_n[e] = 0.0;
+  for (int e = tid; e < KDP * SS * (NWF - 1); e += FINTRI_NT) s_p[e] = 0.0;
   __syncthreads();
-  // ---- 1. N[j][l] = Cp[j] . V[l] for j < l < m
-  for (int jb = warp; jb < KB && 8 * jb < m; jb += FINTRI_NT / 32) {
-    double acc[KB][2];
+  {
+    const int mbn = (m + 7) >> 3;
+    double acc[KB][KB][2];
 #pragma unroll
-    for (int lb = 0; lb < KB; ++lb) acc[lb][0] = acc[lb][1] = 0.0;
-    const bool a_ok = 8 * jb + g < m;
-    const double* ap = Cp + (size_t)(8 * jb + g) * ns + 4 * t;
+    for (int jb = 0; jb < KB; ++jb)
+#pragma unroll
+      for (int lb = 0; lb < KB; ++lb) acc[jb][lb][0] = acc[jb][lb][1] = 0.0;
+    const double* ap = Cp + (size_t)g * ns + 4 * t;
     const double* vp = V + (size_t)g * ns + 4 * t;
-#pragma unroll 2   // two chunks of fragment loads in flight (the loop is a chain of L2 round trips otherwise)
-    for (int s = 0; s < ns; s += 16) {
-      double a[4] = {0.0, 0.0, 0.0, 0.0};
-      if (a_ok) ld32(ap + s, a);
-      double b[KB][4];
+#pragma unroll 2   // two chunks of fragment loads in flight
+    for (int s = 16 * warp; s < ns; s += 16 * NWF) {
+      double a[KB][4], b[KB][4];
 #pragma unroll
-      for (int lb = 0; lb < KB; ++lb) {
-        b[lb][0] = b[lb][1] = b[lb][2] = b[lb][3] = 0.0;
-        if (lb >= jb && 8 * lb + g < m) ld32(vp + (size_t)(8 * lb) * ns + s, b[lb]);
+      for (int jb = 0; jb < KB; ++jb) {
+        a[jb][0] = a[jb][1] = a[jb][2] = a[jb][3] = 0.0;
+        b[jb][0] = b[jb][1] = b[jb][2] = b[jb][3] = 0.0;
+        if (jb < mbn && 8 * jb + g < m) {
+          ld32(ap + (size_t)(8 * jb) * ns + s, a[jb]);
+          ld32(vp + (size_t)(8 * jb) * ns + s, b[jb]);
+        }
       }
 #pragma unroll
       for (int q = 0; q < 4; ++q)
 #pragma unroll
-        for (int lb = 0; lb < KB; ++lb)
-          if (lb >= jb) dmma884(acc[lb], a[q], b[lb][q]);
+        for (int jb = 0; jb < KB; ++jb)
+#pragma unroll
+          for (int lb = jb; lb < KB; ++lb)
+            if (lb < mbn) dmma884(acc[jb][lb], a[jb][q], b[lb][q]);
     }
+    double* dst = warp == 0 ? s_n : s_p + (size_t)(warp - 1) * KDP * SS;
 #pragma unroll
-    for (int lb = 0; lb < KB; ++lb)
+    for (int jb = 0; jb < KB; ++jb)
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int j = 8 * jb + g, l = 8 * lb + 2 * t + e;
-        if (lb >= jb && j < l && l < m) s_n[j * SS + l] = acc[lb][e];
-      }
+      for (int lb = jb; lb < KB; ++lb)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int j = 8 * jb + g, l = 8 * lb + 2 * t + e;
+          if (j < l && l < m) dst[j * SS + l] = acc[jb][lb][e];
+        }
+  }
+  __syncthreads();
+  for (int e = tid; e < KDP * SS; e += FINTRI_NT) {
+    double sum = s_n[e];
+#pragma unroll
+    for (int q = 0; q < NWF - 1; ++q) sum += s_p[(size_t)q * KDP * SS + e];
+    s_n[e] = sum;
   }
   __syncthreads();
   // ---- 2. T = (I + N)^-1: column c solves (I + N) x = e_c from the bottom up; x[l] = 0 below the diagonal
@@ -420,31 +442,43 @@ __global__ void __launch_bounds__(FINTRI_NT, QMC_FINTRI_MIN_CTAS) flush_finalize
     for (int l = 0; l < KDP; ++l) s_t[l * SS + c] = x[l];
   }
   __syncthreads();
-  // ---- 3. Z = T Cp: a warp takes the 16-row strips of Z and 16-column chunks in turn
+  // ---- 3. Z = T Cp: a warp takes the 16-row strips of Z and 16-column chunks in turn; the Cp fragments of its next item
+  // are loaded before the tiles of the current one are multiplied
   constexpr int NSTRIP = KDP >= 16 ? KDP / 16 : 1, RB = KDP >= 16 ? 2 : 1;
   const int mb = (m + 7) >> 3;
-  for (int item = warp; item < NSTRIP * (ns / 16); item += FINTRI_NT / 32) {
+  const int n_items = NSTRIP * (ns / 16);
+  auto load_z = [&](int item, double2 (&z)[KB][2]) {
+    const int j0 = (item / NSTRIP) * 16;
+#pragma unroll
+    for (int b2 = 0; b2 < KB; ++b2)
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        z[b2][q] = make_double2(0.0, 0.0);
+        if (b2 < mb && 8 * b2 + 2 * t + q < m) z[b2][q] = *reinterpret_cast<const double2*>(Cp + (size_t)(8 * b2 + 2 * t + q) * ns + j0 + 2 * g);
+      }
+  };
+  Frag2<KB> f;
+  f.x0[0] = f.x0[1] = f.x0[2] = f.x0[3] = 0.0;
+  f.x1[0] = f.x1[1] = f.x1[2] = f.x1[3] = 0.0;
+  double2 znext[KB][2];
+  if (warp < n_items) load_z(warp, znext);
+  for (int item = warp; item < n_items; item += NWF) {
     const int strip = item % NSTRIP, j0 = (item / NSTRIP) * 16;
+#pragma unroll
+    for (int b2 = 0; b2 < KB; ++b2)
+#pragma unroll
+      for (int q = 0; q < 2; ++q) f.z[b2][q] = znext[b2][q];
+    if (item + NWF < n_items) load_z(item + NWF, znext);
     if (16 * strip >= m) continue;
     // T as the A operand of the strip kernel's GEMM 2: rows 16 strip + 8 i + g, contraction index 8 b + 2 t + e
     double nw[2][KB][2];
 #pragma unroll
     for (int i = 0; i < 2; ++i)
 #pragma unroll
-      for (int b = 0; b < KB; ++b)
+      for (int b2 = 0; b2 < KB; ++b2)
 #pragma unroll
         for (int e = 0; e < 2; ++e)
-          nw[i][b][e] = s_t[(16 * strip + 8 * (i % RB) + g) * SS + 8 * b + 2 * t + e];
-    Frag2<KB> f;
-    f.x0[0] = f.x0[1] = f.x0[2] = f.x0[3] = 0.0;
-    f.x1[0] = f.x1[1] = f.x1[2] = f.x1[3] = 0.0;
-#pragma unroll
-    for (int b = 0; b < KB; ++b)
-#pragma unroll
-      for (int q = 0; q < 2; ++q) {
-        f.z[b][q] = make_double2(0.0, 0.0);
-        if (b < mb && 8 * b + 2 * t + q < m) f.z[b][q] = *reinterpret_cast<const double2*>(Cp + (size_t)(8 * b + 2 * t + q) * ns + j0 + 2 * g);
-      }
+          nw[i][b2][e] = s_t[(16 * strip + 8 * (i % RB) + g) * SS + 8 * b2 + 2 * t + e];
     double* o0 = Z + (size_t)(16 * strip + g) * ns + 4 * t + j0;
     // KDP = 8 has one row block: the second one repeats it (same values to the same addresses)
     mma_store_frag2<KB>(f, nw, mb, o0, RB == 2 ? o0 + (size_t)8 * ns : o0);
