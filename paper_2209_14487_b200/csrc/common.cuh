@@ -261,6 +261,17 @@ __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned
 
 __device__ __forceinline__ double u01(unsigned x) { return ((double)x + 0.5) * (1.0 / 4294967296.0); }
 
+// 32-byte vector access (sm_100: ld/st.global.v4.f64 -> LDG.E.256 / STG.E.256): one L1 request per lane
+// instead of two; p must be 32-byte aligned.
+__device__ __forceinline__ void ld32(const double* p, double (&v)[4])
+{
+  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
+}
+__device__ __forceinline__ void st32(double* p, double a, double b, double c, double d)
+{
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
 // FP64 tensor-core tile: D(8x8) += A(8x4, row) B(4x8, col). Lane l holds A[l/4][l%4],
 // B[l%4][l/4] and D[l/4][2(l%4) + {0,1}].  SASS: DMMA.8x8x4.
 __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b)

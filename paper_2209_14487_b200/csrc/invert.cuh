@@ -137,18 +137,27 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
   double* redv = colf + ns;
   int* redi = reinterpret_cast<int*>(redv + INVB2_NT / 32);
   int* piv = redi + INVB2_NT / 32;
+  int* rsrc = reinterpret_cast<int*>(colf);         // [ns] row sources of the current panel's trailing update
   __shared__ int s_bad;
   double* X = d.Binv + (size_t)blockIdx.x * ns * ns;
   if (tid == 0) s_bad = 0;
   __syncthreads();
+#ifdef QMC_INV_CLOCKS
+  long long ph_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, ph_c = clock64();
+#define IPH(x) do { if (tid == 0) { const long long c_ = clock64(); ph_t[x] += c_ - ph_c; ph_c = c_; } } while (0)
+#else
+#define IPH(x) do {} while (0)
+#endif
   for (int c0 = 0; c0 < n; c0 += INVB_NB) {
     const int nb = min(INVB_NB, n - c0);
     // (a) panel into shared memory (zero padded), eliminated there in place
+#pragma unroll 8   // eight independent loads in flight per thread (the panel load is a latency chain otherwise)
     for (int e = tid; e < ns * INVB_NB; e += INVB2_NT) {
       const int r = e / INVB_NB, j = e - r * INVB_NB;
       XG[r * INVB2_XS + j] = (r < n && j < nb) ? X[(size_t)r * ns + c0 + j] : 0.0;
     }
     __syncthreads();
+    IPH(0);
     // The panel itself is eliminated in sub-panels of INVB_SB columns, the same right-looking scheme one level down:
     // a pivot step touches n x SB elements (a warp takes four rows at a time, lane = (row, sub-panel column), the
     // multiplier of a row is a shuffle, the row interchange is done on register copies of rows c and p, the search
@@ -197,18 +206,21 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
         __syncthreads();   // rows c and p are in registers everywhere; the partial maxima have been read
         double best = -1.0;
         int bi = c + 1;
-        for (int rb = warp * RPW; rb < n; rb += 4 * RPW * NW) {   // warp-uniform trip count; four independent row groups
-          const int r0 = rb + rsub;
+        // a warp pass takes 16 consecutive rows: lane group rsub the rows 4 rsub + i, i = 0..3 in turn.  Rows four apart
+        // sit 8 double-banks apart (row stride 34), so the four groups' 8-column runs tile the 16 double-banks exactly
+        // twice -- two wavefronts per access, the minimum (four with adjacent rows).
+        for (int rb = warp * 4 * RPW; rb < n; rb += 4 * RPW * NW) {   // warp-uniform trip count; four independent rows
+          const int r0 = rb + 4 * rsub;
           double v[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            const int r = r0 + i * RPW * NW;
+            const int r = r0 + i;
             v[i] = (r < n) ? XG[r * INVB2_XS + s0 + col] : 0.0;
             v[i] = (r == p) ? crow : v[i];   // row p receives the old row c
           }
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            const int r = r0 + i * RPW * NW;
+            const int r = r0 + i;
             const double cf = __shfl_sync(0xffffffffu, v[i], lbase + jl);
             double nv = fma(-cf, rc, (col == jl) ? 0.0 : v[i]);
             nv = (r == c) ? rc : nv;
@@ -234,9 +246,10 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
       }
       if (bad) break;
       __syncthreads();   // the sub-panel holds its Gauss-Jordan operator; piv[] of its columns is visible
+      IPH(1);
       if (nb > sb) {
         // the sub-panel's row swaps on the other panel columns (a thread owns a column: no barrier), then its pivot
-        // rows, then the rank-sb update X[:, o] <- X[:, o] + (G - E_K) A_K[:, o]  (rows of K: G[K, :] A_K[:, o])
+        // rows, then the rank-sb update X[:, o] <- X[:, o] + (G - E_K) A_K[:, o]  (rows of K: G[K, :] A_K[:, o]) ...
         if (tid < INVB_NB && (tid < s0 || tid >= s0 + sb)) {
           for (int q = 0; q < sb; ++q) {
             const int c = c0 + s0 + q, p = piv[c];
@@ -249,39 +262,79 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
           for (int q = 0; q < sb; ++q) AKs[q * INVB_NB + tid] = XG[(c0 + s0 + q) * INVB2_XS + tid];
         }
         __syncthreads();
-        const bool other = lane < s0 || lane >= s0 + sb;   // lane = panel column again, a warp owns whole rows
-        double ak[SB];
+        // ... as one FP64 tensor-core GEMM per 16-row tile (k = SB: two MMA k-steps).  Column nn of MMA tile b is panel
+        // column f = ((nn >> 1) & 1) + 16 (nn >> 2) + 4 b + 2 (nn & 1): a lane's accumulator pair (nn = 2 t, 2 t + 1) then
+        // sits at 34 g + (t & 1) + 16 (t >> 1) + const, which tiles the 16 double-banks exactly twice per access (the
+        // shuffle form -- one load, eight shuffles, one store per row -- kept the L1 data pipe three times as busy).
+        const int g = lane >> 2, t = lane & 3;
+        const int fc = (t & 1) + 16 * (t >> 1);                                   // + 4 b + 2 e
+        double bk[2][4];
 #pragma unroll
-        for (int q = 0; q < SB; ++q) ak[q] = (q < sb && other) ? AKs[q * INVB_NB + lane] : 0.0;
-#pragma unroll 2
-        for (int r = warp; r < n; r += NW) {
-          const double x = XG[r * INVB2_XS + lane];
-          const bool in_k = r >= c0 + s0 && r < c0 + s0 + sb;
-          double acc = in_k ? 0.0 : x;
+        for (int q2 = 0; q2 < 2; ++q2)
 #pragma unroll
-          for (int q = 0; q < SB; ++q) acc = fma(__shfl_sync(0xffffffffu, x, s0 + q), ak[q], acc);
-          if (other) XG[r * INVB2_XS + lane] = acc;
+          for (int b2 = 0; b2 < 4; ++b2) {
+            const int k = 4 * q2 + t, col = ((g >> 1) & 1) + 16 * (g >> 2) + 4 * b2 + 2 * (g & 1);
+            bk[q2][b2] = (k < sb && (col < s0 || col >= s0 + sb)) ? AKs[k * INVB_NB + col] : 0.0;
+          }
+        for (int rt = warp; rt < (n + 15) / 16; rt += NW) {
+          double acc[2][4][2];
+          double* xr[2];
+#pragma unroll
+          for (int i = 0; i < 2; ++i) {
+            const int r = rt * 16 + 8 * i + g;
+            const bool in_k = r >= c0 + s0 && r < c0 + s0 + sb;
+            xr[i] = XG + r * INVB2_XS;
+#pragma unroll
+            for (int b2 = 0; b2 < 4; ++b2)
+#pragma unroll
+              for (int e = 0; e < 2; ++e) acc[i][b2][e] = in_k ? 0.0 : xr[i][fc + 4 * b2 + 2 * e];
+          }
+#pragma unroll
+          for (int q2 = 0; q2 < 2; ++q2) {
+            const double a0 = xr[0][s0 + 4 * q2 + t], a1 = xr[1][s0 + 4 * q2 + t];
+#pragma unroll
+            for (int b2 = 0; b2 < 4; ++b2) {
+              dmma884(acc[0][b2], a0, bk[q2][b2]);
+              dmma884(acc[1][b2], a1, bk[q2][b2]);
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int b2 = 0; b2 < 4; ++b2)
+#pragma unroll
+              for (int e = 0; e < 2; ++e) {
+                const int col = fc + 4 * b2 + 2 * e;
+                if (col < s0 || col >= s0 + sb) xr[i][col] = acc[i][b2][e];
+              }
         }
         __syncthreads();
       }
+      IPH(2);
     }
     if (bad && tid == 0) s_bad = 1;
+    // (b) the panel's row swaps on the columns outside the panel are not carried out as swaps: rsrc[r] = the row whose
+    // content they move to position r, and the trailing update below reads row rsrc[r] where it writes row r.  Every
+    // swap pairs a row of K with a pivot row, so a pivot row's position only ever receives old rows of K; a warp owns
+    // its 16 columns, reads the (permuted) rows of K first and writes them last: no row is read after it was written.
+    // (As a pass of its own -- 32 dependent load/store pairs per column -- the swaps were 14 % of the kernel; issued
+    // from the pivot steps they stalled the pivot chain on their loads.)
+    for (int r = tid; r < ns; r += INVB2_NT) rsrc[r] = r;
+    __syncthreads();
+    if (tid == 0 && !s_bad)
+      for (int j = 0; j < nb; ++j) {
+        const int c = c0 + j, pp = piv[c], x = rsrc[c];
+        rsrc[c] = rsrc[pp];
+        rsrc[pp] = x;
+      }
     __syncthreads();
     if (s_bad) break;
-    // (b) the panel's row swaps on every other column (a thread owns whole columns: no barrier needed)
-    for (int o = tid; o < n; o += INVB2_NT) {
-      if (o >= c0 && o < c0 + nb) continue;
-      for (int j = 0; j < nb; ++j) {
-        const int c = c0 + j, p = piv[c];
-        if (p != c) {
-          const double a = X[(size_t)c * ns + o], b = X[(size_t)p * ns + o];
-          X[(size_t)c * ns + o] = b;
-          X[(size_t)p * ns + o] = a;
-        }
-      }
-    }
-    __syncthreads();
-    // (d) trailing update by 16-column blocks: A[:, o] <- A[:, o] + (X_G - E_K) A_K[:, o], rows of K last
+    IPH(3);
+    // (d) trailing update by 16-column blocks: A[:, o] <- A[:, o] + (X_G - E_K) A_K[:, o], rows of K last.
+    // The column index of an MMA result may be permuted freely if the B operand uses the same permutation: column nn of
+    // tile b is column 4 (nn / 2) + 2 b + (nn % 2) of the block, so a lane's two tiles are four consecutive columns -- one
+    // 32-byte load and one 32-byte store per row, four lanes covering one 128-byte line (8-byte stores and 16-byte loads
+    // of half lines made the L1 data pipe the busiest unit of this kernel: ncu r2).
     {
       const int g = lane >> 2, t = lane & 3;
       const int ncb = (n + 15) / 16, nrt = (n + 31) / 32;
@@ -293,25 +346,38 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
         for (int q = 0; q < INVB_NB / 4; ++q)
 #pragma unroll
           for (int b = 0; b < 2; ++b) {
-            const int j = 4 * q + t, o = o0 + 8 * b + g;
-            bb[q][b] = (j < nb && o < n) ? X[(size_t)(c0 + j) * ns + o] : 0.0;
+            const int j = 4 * q + t, o = o0 + 4 * (g >> 1) + 2 * b + (g & 1);
+            bb[q][b] = (j < nb && o < n) ? X[(size_t)rsrc[c0 + j] * ns + o] : 0.0;
           }
-        for (int rt = 0; rt <= nrt; ++rt) {
-          // row tiles in order with the tile of K skipped, then the tile of K
-          const bool in_k = rt == nrt;
-          const int r0 = in_k ? c0 : rt * 32;
-          if (!in_k && r0 == c0) continue;
+        // row tiles in order with the tile of K skipped, then the tile of K (its rows of X are not read: acc = 0); the
+        // loads of the next tile are issued before the current tile's 64 MMAs, so a warp overlaps its own memory latency
+        auto tile_r0 = [&](int rt) { return rt == nrt ? c0 : rt * 32; };
+        auto tile_load = [&](int rt, double (&x)[4][4]) {
+          const int r0 = tile_r0(rt);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int r = r0 + 8 * i + g;
+            x[i][0] = x[i][1] = x[i][2] = x[i][3] = 0.0;
+            if (rt < nrt && r < n) ld32(X + (size_t)rsrc[r] * ns + o0 + 4 * t, x[i]);
+          }
+        };
+        const int rt_first = c0 == 0 ? 1 : 0;
+        double xn[4][4];
+        tile_load(rt_first, xn);
+        for (int rt = rt_first; rt <= nrt; ++rt) {
+          if (rt < nrt && rt * 32 == c0) continue;
+          const int r0 = tile_r0(rt);
           double acc[4][2][2];
 #pragma unroll
           for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int b = 0; b < 2; ++b) {
-              const int r = r0 + 8 * i + g, o = o0 + 8 * b + 2 * t;
-              double2 x = make_double2(0.0, 0.0);
-              if (!in_k && r < n && o < ns) x = *reinterpret_cast<const double2*>(X + (size_t)r * ns + o);
-              acc[i][b][0] = x.x;
-              acc[i][b][1] = x.y;
+              acc[i][b][0] = xn[i][2 * b];
+              acc[i][b][1] = xn[i][2 * b + 1];
             }
+          int rn = rt + 1;
+          if (rn < nrt && rn * 32 == c0) ++rn;
+          if (rn <= nrt) tile_load(rn, xn);
 #pragma unroll
           for (int q = 0; q < INVB_NB / 4; ++q) {
             double a[4];
@@ -323,15 +389,10 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
               for (int b = 0; b < 2; ++b) dmma884(acc[i][b], a[i], bb[q][b]);
           }
 #pragma unroll
-          for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int b = 0; b < 2; ++b) {
-              const int r = r0 + 8 * i + g, o = o0 + 8 * b + 2 * t;
-              if (r < n) {
-                if (o < n) X[(size_t)r * ns + o] = acc[i][b][0];
-                if (o + 1 < n) X[(size_t)r * ns + o + 1] = acc[i][b][1];
-              }
-            }
+          for (int i = 0; i < 4; ++i) {
+            const int r = r0 + 8 * i + g;   // (padding columns o >= n receive the zeros they already hold)
+            if (r < n) st32(X + (size_t)r * ns + o0 + 4 * t, acc[i][0][0], acc[i][0][1], acc[i][1][0], acc[i][1][1]);
+          }
         }
       }
     }
@@ -341,6 +402,7 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
       X[(size_t)r * ns + c0 + j] = XG[r * INVB2_XS + j];
     }
     __syncthreads();
+    IPH(4);
   }
   if (s_bad) {
     if (tid == 0) atomicExch(d.status, 4);
@@ -365,6 +427,12 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
     for (int j = lane; j < n; j += 32) X[(size_t)r * ns + j] = rowbuf[src[j]];
     __syncwarp();
   }
+#ifdef QMC_INV_CLOCKS
+  __syncthreads();
+  IPH(5);
+  if (tid == 0)
+    for (int q = 0; q < 8; ++q) d.pvec[(size_t)blockIdx.x * 8 + q] = (double)ph_t[q];
+#endif
 }
 
 // D:R6: dst = fl32(src), four elements per thread (total % 4 == 0: ns is a multiple of 16)

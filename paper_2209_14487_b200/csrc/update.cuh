@@ -146,17 +146,6 @@ constexpr int FLUSH_NT = QMC_FLUSH_NT;    // one 16-row strip per warp
 constexpr int FLUSH_ROWS_PER_WARP = 16;  // two 8-row MMA blocks
 constexpr int FINALIZE_NT = 128;
 
-// 32-byte vector access (sm_100: ld/st.global.v4.f64 -> LDG.E.256 / STG.E.256): one L1 request per lane
-// instead of two; p must be 32-byte aligned.
-__device__ __forceinline__ void ld32(const double* p, double (&v)[4])
-{
-  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
-}
-__device__ __forceinline__ void st32(double* p, double a, double b, double c, double d)
-{
-  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-}
-
 // Four consecutive elements of the carried inverse in its storage type (D:R6): fp64, or fp32 widened on load and
 // rounded to nearest on store.
 __device__ __forceinline__ void ld_b4(const double* p, double (&v)[4]) { ld32(p, v); }
