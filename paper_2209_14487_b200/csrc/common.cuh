@@ -261,6 +261,14 @@ __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned
 
 __device__ __forceinline__ double u01(unsigned x) { return ((double)x + 0.5) * (1.0 / 4294967296.0); }
 
+// 16-byte asynchronous copy global -> shared through L2 only (L1 is not involved).  SASS: LDGSTS.
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
+{
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // 32-byte vector access (sm_100: ld/st.global.v4.f64 -> LDG.E.256 / STG.E.256): one L1 request per lane
 // instead of two; p must be 32-byte aligned.
 __device__ __forceinline__ void ld32(const double* p, double (&v)[4])

@@ -234,7 +234,9 @@ int launch_build_t(qmc_crowd* c)
     order = ord;
   }
 #endif
-  spline_build_kernel<T><<<(unsigned)blocks, SPLINE_NT, smem, c->stream>>>(d, order);
+  if (order)
+    spline_build_cells_kernel<T><<<(unsigned)(d.grid[0] * d.grid[1] * d.grid[2]), BUILD_NT, BUILD_SMEM, c->stream>>>(d, order, d.cell_bins);
+  else spline_build_kernel<T><<<(unsigned)blocks, SPLINE_NT, smem, c->stream>>>(d);
   LAUNCH_CHECK(c);
   if (order) {   // the sorted build writes A row-major: transpose to the A^T the inversion expects
     transpose_inplace_kernel<<<dim3((unsigned)(d.ns / 16), (unsigned)(2 * d.W)), 256, 0, c->stream>>>(d);
@@ -253,7 +255,11 @@ int rebuild(qmc_crowd* c)
   c->launches += 3;
   int st = c->is_f64 ? launch_build_t<double>(c) : launch_build_t<float>(c);
   if (st) return st;
+#ifdef QMC_INV_PAD_SMEM
+  const size_t b2smem = invert_blocked2_smem(d.ns) + QMC_INV_PAD_SMEM;
+#else
   const size_t b2smem = invert_blocked2_smem(d.ns);
+#endif
   if (b2smem <= 227 * 1024 && d.ns <= 2 * INVB2_NT) {
     invert_blocked2_kernel<<<(unsigned)(d.W * 2), INVB2_NT, b2smem, c->stream>>>(d);
   } else {
@@ -488,7 +494,8 @@ cudaError_t raise_smem_limits_t(int optin)
                        (const void*)window_kernel<T, 128, 0, float>, (const void*)window_kernel<T, 256, 0, float>,
                        (const void*)window_kernel<T, 512, 0, float>,
                        (const void*)window_kernel<T, 256>, (const void*)window_kernel<T, 512>,
-                       (const void*)sweep1_kernel<T>, (const void*)spline_build_kernel<T>, (const void*)kinetic_kernel<T>};
+                       (const void*)sweep1_kernel<T>, (const void*)spline_build_kernel<T>, (const void*)spline_build_cells_kernel<T>,
+                       (const void*)kinetic_kernel<T>};
   for (const void* f : fns) {
     cudaError_t e = raise_smem_limit(f, optin);
     if (e != cudaSuccess) return e;

@@ -179,6 +179,33 @@ __device__ __forceinline__ void spline_plane_sum(const SplineW<float>& s, int a,
 __device__ __forceinline__ float shfl_xor_t(float v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 __device__ __forceinline__ double shfl_xor_t(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 
+// Sum over the four planes (lanes 8 a + slice) with the owner of each quantity as the only receiver: plane a's lane ends
+// up with quantity a of the slice (f0), plane 0's also with the laplacian (f1).  Same pairwise tree per value as two full
+// xor-shuffles, (p_a + p_{a^1}) + (p_{a^2} + p_{a^3}), with 5 instead of 10 shuffles per value.
+template <typename T>
+__device__ __forceinline__ void spline_plane_reduce(int a, const T (&out)[5][Vec16<T>::W], T (&f0)[Vec16<T>::W], T (&f1)[Vec16<T>::W])
+{
+  constexpr int VW = Vec16<T>::W;
+  const bool odd = a & 1, up = a & 2;
+  T r0[VW], r1[VW], r2[VW];  // after step 1: even lanes hold q0, q2, q4; odd lanes hold q1, q3 (r2 unused)
+#pragma unroll
+  for (int e = 0; e < VW; ++e) {
+    const T s0 = odd ? out[0][e] : out[1][e], s1 = odd ? out[2][e] : out[3][e], s2 = odd ? out[4][e] : (T)0;
+    const T k0 = odd ? out[1][e] : out[0][e], k1 = odd ? out[3][e] : out[2][e], k2 = out[4][e];
+    r0[e] = k0 + shfl_xor_t(s0, 8);
+    r1[e] = k1 + shfl_xor_t(s1, 8);
+    r2[e] = k2 + shfl_xor_t(s2, 8);
+  }
+  // after step 2: plane 0: q0, q4; plane 1: q1; plane 2: q2; plane 3: q3
+#pragma unroll
+  for (int e = 0; e < VW; ++e) {
+    const T s0 = up ? r0[e] : r1[e], s1 = up ? r2[e] : (T)0;
+    const T k0 = up ? r1[e] : r0[e], k1 = r2[e];
+    f0[e] = k0 + shfl_xor_t(s0, 16);
+    f1[e] = k1 + shfl_xor_t(s1, 16);
+  }
+}
+
 // All orbitals at position r by the whole CTA (NT threads, NT % 32 == 0).  `s` is shared memory;
 // `vgl` (global or shared) receives [5][ns]: phi, d/dx, d/dy, d/dz, laplacian, zero beyond M.
 // Contains two __syncthreads(); must be called by all threads of the CTA.
@@ -222,27 +249,8 @@ __device__ __forceinline__ void spline_cta(const CrowdDev& d, const double* r, S
 #pragma unroll
         for (int e = 0; e < VW; ++e) out[q][e] = (T)0;
     }
-    // Sum over the four planes (lanes 8 a + slice) with the owner of each quantity as the only receiver: plane a's lane
-    // ends up with quantity a, plane 0's also with the laplacian.  Same pairwise tree per value as two full xor-shuffles,
-    // (p_a + p_{a^1}) + (p_{a^2} + p_{a^3}), with 5 instead of 10 shuffles per value.
-    const bool odd = a & 1, up = a & 2;
-    T r0[VW], r1[VW], r2[VW];  // after step 1: even lanes hold q0, q2, q4; odd lanes hold q1, q3 (r2 unused)
-#pragma unroll
-    for (int e = 0; e < VW; ++e) {
-      const T s0 = odd ? out[0][e] : out[1][e], s1 = odd ? out[2][e] : out[3][e], s2 = odd ? out[4][e] : (T)0;
-      const T k0 = odd ? out[1][e] : out[0][e], k1 = odd ? out[3][e] : out[2][e], k2 = out[4][e];
-      r0[e] = k0 + shfl_xor_t(s0, 8);
-      r1[e] = k1 + shfl_xor_t(s1, 8);
-      r2[e] = k2 + shfl_xor_t(s2, 8);
-    }
-    T f0[VW], f1[VW];  // after step 2: lane 0: q0, q4; lane 1: q1; lane 2: q2; lane 3: q3
-#pragma unroll
-    for (int e = 0; e < VW; ++e) {
-      const T s0 = up ? r0[e] : r1[e], s1 = up ? r2[e] : (T)0;
-      const T k0 = up ? r1[e] : r0[e], k1 = r2[e];
-      f0[e] = k0 + shfl_xor_t(s0, 16);
-      f1[e] = k1 + shfl_xor_t(s1, 16);
-    }
+    T f0[VW], f1[VW];
+    spline_plane_reduce<T>(a, out, f0, f1);
 #pragma unroll
     for (int e = 0; e < VW; ++e)
       if (!FULL && (int)(chunk * VW) + e >= sh_M<NS>(d)) f0[e] = f1[e] = (T)0;
@@ -265,34 +273,25 @@ __global__ void __launch_bounds__(SPLINE_NT, 4) spline_vgl_kernel(CrowdDev d)
   spline_cta<T, SPLINE_NT>(d, d.rnew + 3 * (size_t)w, s, static_cast<T*>(d.vgl) + (size_t)w * 5 * d.ns);
 }
 
-// qmc_crowd_create / set_positions: one CTA per (walker, electron) at the electron's own position;
-// fills the caches and the transposed Slater matrix X[j][i] = phi_j(r_i) that the inversion kernel
-// turns into B = (A^-1)^T = (A^T)^-1 (D:C2).  dynamic smem: 5 ns elements of T.
-// order != nullptr: CTA b takes (walker, electron) order[b] -- the positions sorted by grid cell (below), so that CTAs
-// in flight together gather overlapping stencils and the table is streamed from DRAM about once instead of once per
-// position (308 GB at cfg 5, W = 4096); the loads then keep their lines in L2.  CTAs of one walker are then no longer
-// neighbours in time, so the Slater matrix is written row-major (A, one contiguous row per electron: the strided
-// 8-byte writes of A^T would stop merging in L2) and transposed in place afterwards (transpose_inplace_kernel).
+// qmc_crowd_create / set_positions on small crowds (fewer than 256 positions; larger ones take the cell-sorted build
+// below): one CTA per (walker, electron) at the electron's own position; fills the caches and the transposed Slater
+// matrix X[j][i] = phi_j(r_i) that the inversion kernel turns into B = (A^-1)^T = (A^T)^-1 (D:C2).
+// dynamic smem: 5 ns elements of T.
 template <typename T>
-__global__ void __launch_bounds__(SPLINE_NT, 4) spline_build_kernel(CrowdDev d, const int* __restrict__ order)
+__global__ void __launch_bounds__(SPLINE_NT, 4) spline_build_kernel(CrowdDev d)
 {
   extern __shared__ double sm_build[];
   __shared__ SplineW<T> s;
   T* v_s = reinterpret_cast<T*>(sm_build);
-  const size_t we = order ? (size_t)order[blockIdx.x] : (size_t)blockIdx.x;
+  const size_t we = (size_t)blockIdx.x;
   const int w = (int)(we / d.N), e_idx = (int)(we - (size_t)w * d.N);
-  if (order) spline_cta<T, SPLINE_NT, NoSideWork, true>(d, d.R + 3 * we, s, v_s);
-  else spline_cta<T, SPLINE_NT>(d, d.R + 3 * we, s, v_s);
+  spline_cta<T, SPLINE_NT>(d, d.R + 3 * we, s, v_s);
   __syncthreads();
   const int spin = e_idx / d.n, i = e_idx - spin * d.n;
   T* cache = static_cast<T*>(d.cache) + we * 4 * d.ns;
   double* X = d.Binv + ((size_t)w * 2 + spin) * d.ns * d.ns;
   for (int j = threadIdx.x; j < 4 * d.ns; j += SPLINE_NT) cache[j] = v_s[d.ns + j];
-  if (order) {
-    for (int j = threadIdx.x; j < d.M; j += SPLINE_NT) X[(size_t)i * d.ns + j] = (double)v_s[j];
-  } else {
-    for (int j = threadIdx.x; j < d.M; j += SPLINE_NT) X[(size_t)j * d.ns + i] = (double)v_s[j];
-  }
+  for (int j = threadIdx.x; j < d.M; j += SPLINE_NT) X[(size_t)j * d.ns + i] = (double)v_s[j];
 }
 
 // X <- X^T for every ns x ns matrix of the crowd, in place: CTA (a, matrix) swaps the 16 x 16 tiles (a, b) and (b, a)
@@ -357,6 +356,130 @@ __global__ void cell_scatter_kernel(CrowdDev d, int* bins, int* order)
 {
   const size_t we = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (we < (size_t)d.W * d.N) order[atomicAdd(bins + cell_of(d, d.R + 3 * we), 1)] = (int)we;
+}
+
+// The Slater build over positions sorted by grid cell (qmc_crowd_create / set_positions / recompute on crowds of 256
+// positions and more).  CTAs in flight together gather overlapping stencils, so the table is streamed from DRAM about
+// once instead of once per position, and the positions of one cell share their 64 stencil rows outright: the CTA of a
+// cell (grid = cells; its range in `order` is bins[cell - 1] .. bins[cell] after the scatter; empty cells exit) takes its
+// positions in runs of up to BUILD_RUN, stages the 64 rows in shared memory ONCE per run (in column segments of
+// BUILD_SEG_BYTES per row: 96 KB, two CTAs per SM) and evaluates every position of the run from there -- a thread takes
+// one 16-byte orbital slice of one position through all four x-planes, so the planes are summed in registers.  At cfg 5,
+// W = 4096 a cell holds 6 positions on average: against one CTA per position with the planes spread over lanes (the
+// form the move kernels use, where a position is evaluated alone) the L2 -> SM traffic falls from 308 GB to 50 GB and the
+// instruction count by 2.4 (no shuffle tree, weights read once per four planes).  Same arithmetic per value as
+// spline_cta -- the same plane sums, added as (p0 + p1) + (p2 + p3) like its shuffle tree -- so the results are
+// bit-identical to the per-position form.  The outputs go straight to global memory: the caches [4][ns] and row i of the
+// row-major Slater matrix A (one contiguous row per electron -- the CTAs of one walker are not neighbours in time,
+// strided 8-byte writes of A^T would not merge in L2 -- transposed in place afterwards by transpose_inplace_kernel).
+// A position whose stencil offsets differ from the run's first (the cell index and the spline's own floor are computed
+// differently and may disagree on a cell face) starts a new sub-run with its own staging.
+constexpr int BUILD_RUN = 16;
+constexpr int BUILD_NT = 192;
+constexpr int BUILD_SEG_BYTES = 1536;
+constexpr size_t BUILD_SMEM = (size_t)64 * BUILD_SEG_BYTES;
+
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ void st_phi_row(double* x, const float (&f)[4]) { st32(x, (double)f[0], (double)f[1], (double)f[2], (double)f[3]); }
+__device__ __forceinline__ void st_phi_row(double* x, const double (&f)[2]) { *reinterpret_cast<double2*>(x) = make_double2(f[0], f[1]); }
+
+template <typename T>
+__global__ void __launch_bounds__(BUILD_NT, 2) spline_build_cells_kernel(CrowdDev d, const int* __restrict__ order,
+                                                                         const int* __restrict__ bins)
+{
+  constexpr int VW = Vec16<T>::W, NT = BUILD_NT;
+  constexpr unsigned SEGV = BUILD_SEG_BYTES / 16;   // 16-byte vectors per staged row
+  constexpr int PP = NT / SEGV;                     // positions evaluated side by side
+  static_assert(NT % SEGV == 0 && PP >= 1, "a thread owns one slice of the segment");
+  extern __shared__ __align__(16) unsigned char sm_cells[];
+  T* st = reinterpret_cast<T*>(sm_cells);           // [64][SEGV * VW]
+  __shared__ SplineW<T> sw[BUILD_RUN];
+  __shared__ double* s_x[BUILD_RUN];                // row i of the position's Slater matrix
+  __shared__ T* s_cache[BUILD_RUN];
+  const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int start = cell ? bins[cell - 1] : 0, end = bins[cell];   // the cell's range in `order` (after the scatter)
+  const T* tab = static_cast<const T*>(d.coefs);
+  const unsigned chunks = (unsigned)d.ns / VW;
+  const unsigned v = tid % SEGV;
+  const int jp = tid / SEGV;
+  for (int b0 = start; b0 < end; b0 += BUILD_RUN) {
+    const int cnt = min(BUILD_RUN, end - b0);
+    __syncthreads();   // the previous run's weights are no longer read
+    if (tid < 3 * cnt) {
+      const int j = tid / 3, c = tid - 3 * j;
+      const size_t we = (size_t)order[b0 + j];
+      spline_axis<T>(d, c, d.R[3 * we + c], sw[j]);
+      if (c == 0) {
+        const int w = (int)(we / d.N), e_idx = (int)(we - (size_t)w * d.N);
+        const int spin = e_idx / d.n, i = e_idx - spin * d.n;
+        s_x[j] = d.Binv + ((size_t)w * 2 + spin) * d.ns * d.ns + (size_t)i * d.ns;
+        s_cache[j] = static_cast<T*>(d.cache) + we * 4 * d.ns;
+      }
+    }
+    __syncthreads();
+    for (int q = 0; q < cnt;) {
+      int qe = q + 1;
+      while (qe < cnt && sw[qe].off[0][0] == sw[q].off[0][0] && sw[qe].off[1][0] == sw[q].off[1][0] &&
+             sw[qe].off[2][0] == sw[q].off[2][0])
+        ++qe;
+      for (unsigned v0 = 0; v0 < chunks; v0 += SEGV) {
+        const unsigned nv = min(SEGV, chunks - v0);
+        __syncthreads();   // the readers of the previous segment are done
+        for (int row = warp; row < 64; row += NT / 32) {   // a warp stages whole rows: contiguous 16-byte pieces
+          const unsigned src0 = sw[q].off[0][row >> 4] + sw[q].off[1][(row >> 2) & 3] + sw[q].off[2][row & 3] + v0;
+          for (unsigned vv = lane; vv < nv; vv += 32) {
+            T* dst = st + ((size_t)row * SEGV + vv) * VW;
+            if (v0 + vv < d.tab_vecs) {
+              cp_async16(dst, tab + (size_t)(src0 + vv) * VW);
+            } else {
+#pragma unroll
+              for (int e = 0; e < VW; ++e) dst[e] = (T)0;   // columns the table does not hold (all >= M: masked below)
+            }
+          }
+        }
+        cp_async_wait_all();
+        __syncthreads();
+        if (v < nv) {
+          const unsigned chunk = v0 + v;
+          for (int j = q + jp; j < qe; j += PP) {
+            const SplineW<T>& s = sw[j];
+            T o01[5][VW], o2[5][VW], res[5][VW];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+              T p[4][4][VW], o[5][VW];
+#pragma unroll
+              for (int bb = 0; bb < 4; ++bb)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                  const T* src = st + ((size_t)(16 * a + 4 * bb + c) * SEGV + v) * VW;
+#pragma unroll
+                  for (int e = 0; e < VW; ++e) p[bb][c][e] = src[e];
+                }
+              spline_plane_sum(s, a, p, o);
+#pragma unroll
+              for (int k = 0; k < 5; ++k)
+#pragma unroll
+                for (int e = 0; e < VW; ++e) {
+                  if (a == 0) o01[k][e] = o[k][e];
+                  if (a == 1) o01[k][e] = add_rn(o01[k][e], o[k][e]);   // (never contracted with the products behind o)
+                  if (a == 2) o2[k][e] = o[k][e];
+                  if (a == 3) res[k][e] = add_rn(o01[k][e], add_rn(o2[k][e], o[k][e]));
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < VW; ++e)
+              if ((int)(chunk * VW) + e >= d.M) res[0][e] = res[1][e] = res[2][e] = res[3][e] = res[4][e] = (T)0;
+            st_phi_row(s_x[j] + (size_t)chunk * VW, res[0]);
+            T* cache = s_cache[j] + (size_t)chunk * VW;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) st16(cache + (size_t)k * d.ns, res[k + 1]);
+          }
+        }
+      }
+      q = qe;
+    }
+  }
 }
 
 }  // namespace qmc

@@ -62,14 +62,6 @@ __device__ __forceinline__ double2 ld_x2(const float* v, int jj)
 }
 __device__ __forceinline__ double2 ld_x2(const double* v, int jj) { return reinterpret_cast<const double2*>(v)[jj]; }
 
-// 16-byte asynchronous copy global -> shared through L2 only (the sources are lines this CTA or the flush
-// wrote earlier; L1 is not involved).  SASS: LDGSTS.
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
-{
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // nbytes % 16 == 0, both 16-byte aligned; strided over the CTA
 template <int NT = MOVE_NT>
 __device__ __forceinline__ void cp_async_cta(void* smem, const void* gmem, int nbytes)
