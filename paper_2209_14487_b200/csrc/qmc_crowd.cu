@@ -255,11 +255,7 @@ int rebuild(qmc_crowd* c)
   c->launches += 3;
   int st = c->is_f64 ? launch_build_t<double>(c) : launch_build_t<float>(c);
   if (st) return st;
-#ifdef QMC_INV_PAD_SMEM
-  const size_t b2smem = invert_blocked2_smem(d.ns) + QMC_INV_PAD_SMEM;
-#else
   const size_t b2smem = invert_blocked2_smem(d.ns);
-#endif
   if (b2smem <= 227 * 1024 && d.ns <= 2 * INVB2_NT) {
     invert_blocked2_kernel<<<(unsigned)(d.W * 2), INVB2_NT, b2smem, c->stream>>>(d);
   } else {
