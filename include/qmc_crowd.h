@@ -245,6 +245,28 @@ enum {
  * are HOST arrays of QMC_N_KERNEL_CLASSES entries (either may be NULL).                       */
 int qmc_crowd_get_profile(qmc_crowd_t* crowd, double* ms, uint64_t* count);
 
+/* ---- an entry point that allocates nothing and needs no crowd and no workspace -------------------
+ * For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the orbital evaluation of qmc_spo_vgl step (c) -- D:C1, the 4x4x4 tricubic B-spline stencil, value /
+ * gradient / laplacian of all M orbitals -- at n_pos caller-given positions, with the kernel's internal result buffer
+ * ([n_pos][5][ns] table elements, ns = M rounded up to 16) in a file-scope `static __device__` array of
+ * QMC_STATIC_SCRATCH_BYTES instead of a workspace.  Every GPU that loads the library holds that array until exit.
+ *   n_orb, grid, box, coef_dtype, coefs_dev, orb_stride: the table, as in qmc_crowd_desc (coefs_dev DEVICE, BORROWED);
+ *   r_dev:  DEVICE [n_pos][3] fp64, not wrapped (periodicity comes from the index arithmetic, D:C1);
+ *   phi / dphi / d2phi: optional DEVICE outputs (NULL to skip), element type = table type, compact layouts
+ *           [n_pos][M], [n_pos][3][M], [n_pos][M] -- the layouts and the values of qmc_spo_vgl's outputs;
+ *   stream: cudaStream_t, BORROWED; the call is asynchronous on it.
+ * Returns QMC_ERR_WORKSPACE (and launches nothing) when n_pos * 5 * ns * sizeof(element) exceeds
+ * QMC_STATIC_SCRATCH_BYTES, QMC_ERR_INVALID_ARG for a malformed table description or NULL inputs; n_pos == 0 is a no-op.
+ * Calls no cudaMalloc / cudaFree and no allocating library routine (the first call on a device looks the array's device
+ * address up with cudaGetSymbolAddress, once per device).  ALL calls of a process on one device share the one array:
+ * calls that overlap on the GPU (different streams, or graphs replayed concurrently) race; serialise them.  The array
+ * keeps the last call's contents; every element a call reads it has written itself first, so nothing needs clearing. */
+#define QMC_STATIC_SCRATCH_BYTES (4u << 20)
+int qmc_spo_vgl_static(int32_t n_orb, const int32_t* grid /*[3]*/, const double* box /*[3]*/, int32_t coef_dtype,
+                       const void* coefs_dev, int64_t orb_stride, int32_t n_pos, const double* r_dev,
+                       void* phi, void* dphi, void* d2phi, void* stream);
+
 const char* qmc_last_error(void); /* thread-local, never NULL */
 const char* qmc_version(void);
 

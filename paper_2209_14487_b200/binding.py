@@ -28,7 +28,9 @@ EXPORTS = [
     "qmc_crowd_set_positions", "qmc_crowd_get_inverse", "qmc_crowd_set_inverse", "qmc_crowd_get_caches",
     "qmc_crowd_get_window", "qmc_crowd_get_move", "qmc_crowd_set_sweep_index", "qmc_crowd_stats",
     "qmc_crowd_launch_count", "qmc_crowd_set_option", "qmc_crowd_get_profile", "qmc_last_error", "qmc_version",
+    "qmc_spo_vgl_static",
 ]
+STATIC_SCRATCH_BYTES = 4 << 20      # QMC_STATIC_SCRATCH_BYTES of include/qmc_crowd.h
 
 
 class QmcError(RuntimeError):
@@ -95,6 +97,7 @@ def load():
     L.qmc_crowd_launch_count.restype = C.c_uint64
     L.qmc_crowd_set_option.argtypes = [vp, ip, ip]
     L.qmc_crowd_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+    L.qmc_spo_vgl_static.argtypes = [ip, C.POINTER(C.c_int32), C.POINTER(C.c_double), ip, vp, C.c_int64, ip, dp, vp, vp, vp, vp]
     L.qmc_last_error.restype = C.c_char_p
     L.qmc_version.restype = C.c_char_p
     _lib = L
@@ -113,6 +116,32 @@ def _ptr(t, dtype=None):
     if dtype is not None:
         assert t.dtype == dtype, (t.dtype, dtype)
     return t.data_ptr()
+
+
+def qmc_spo_vgl_static(coefs, box, r, phi=None, dphi=None, d2phi=None):
+    """include/qmc_crowd.h qmc_spo_vgl_static: orbitals at the positions r [P][3] (CUDA fp64) from the table coefs
+    [gx][gy][gz][orb_stride] (CUDA fp32 / fp64, n_orb = orb_stride), no crowd, no workspace, no allocation inside the
+    library.  phi [P][M], dphi [P][3][M], d2phi [P][M]: caller-owned CUDA outputs of the table's dtype (allocated here
+    when None -- by the caller's allocator, outside the library).  Runs on the current stream."""
+    import torch
+    assert coefs.is_cuda and coefs.is_contiguous() and coefs.dim() == 4 and r.is_cuda and r.dtype == torch.float64
+    r = r.contiguous()
+    P, M = int(r.shape[0]), int(coefs.shape[3])
+    grid = (C.c_int32 * 3)(*[int(x) for x in coefs.shape[:3]])
+    bx = (C.c_double * 3)(*([float(box)] * 3 if not hasattr(box, "__len__") else [float(x) for x in box]))
+    if phi is None:
+        phi = torch.empty((P, M), dtype=coefs.dtype, device=coefs.device)
+    if dphi is None:
+        dphi = torch.empty((P, 3, M), dtype=coefs.dtype, device=coefs.device)
+    if d2phi is None:
+        d2phi = torch.empty((P, M), dtype=coefs.dtype, device=coefs.device)
+    for o in (phi, dphi, d2phi):
+        assert o.is_cuda and o.is_contiguous() and o.dtype == coefs.dtype
+    stream = torch.cuda.current_stream(coefs.device).cuda_stream
+    _check(load().qmc_spo_vgl_static(M, grid, bx, 1 if coefs.dtype == torch.float64 else 0, coefs.data_ptr(), M, P,
+                                     r.data_ptr() if P else None, phi.data_ptr() if P else None,
+                                     dphi.data_ptr() if P else None, d2phi.data_ptr() if P else None, stream))
+    return phi, dphi, d2phi
 
 
 class Crowd:

@@ -9,6 +9,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1142,3 +1143,107 @@ int qmc_crowd_set_option(qmc_crowd_t* c, int option, int value)
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// qmc_spo_vgl_static: the orbital evaluation with its scratch in a static device array (include/qmc_crowd.h)
+// ------------------------------------------------------------------------------------------
+namespace {
+
+// The internal [n_pos][5][ns] result buffer of the spline kernel (what d.vgl is in a crowd's workspace).  In HOST code
+// this name is a host-side stand-in, not a device address: host code uses static_scratch_address() below.
+static __device__ __align__(256) unsigned char g_static_scratch[QMC_STATIC_SCRATCH_BYTES];
+
+// Variant of spline_vgl_kernel: one CTA per position r[b], result into vgl[b] (the static array), no crowd state.
+template <typename T>
+__global__ void __launch_bounds__(qmc::SPLINE_NT, 4) spline_vgl_static_kernel(qmc::CrowdDev d, const double* __restrict__ r,
+                                                                              T* __restrict__ vgl)
+{
+  __shared__ qmc::SplineW<T> s;
+  const size_t b = blockIdx.x;
+  qmc::spline_cta<T, qmc::SPLINE_NT>(d, r + 3 * b, s, vgl + b * 5 * d.ns);
+}
+
+// Device address of g_static_scratch on the current device: looked up once per device, with that device current.
+int static_scratch_address(void** out)
+{
+  static void* addr[64] = {};
+  static std::mutex mu;
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(QMC_ERR_INVALID_ARG, "device ordinal %d out of range", dev);
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress(&p, g_static_scratch));
+    if (!p) return fail(QMC_ERR_CUDA, "cudaGetSymbolAddress returned a null address for the static scratch");
+    addr[dev] = p;
+  }
+  *out = addr[dev];
+  return QMC_OK;
+}
+
+template <typename T>
+int spo_vgl_static_t(const qmc::CrowdDev& d, int n_pos, const double* r_dev, T* vgl, T* phi, T* dphi, T* d2phi, cudaStream_t stream)
+{
+  spline_vgl_static_kernel<T><<<(unsigned)n_pos, qmc::SPLINE_NT, 0, stream>>>(d, r_dev, vgl);
+  const size_t ns = (size_t)d.ns;
+  struct Out { T* dst; const T* src; int rows; } outs[3] = {{phi, vgl, 1}, {dphi, vgl + ns, 3}, {d2phi, vgl + 4 * ns, 1}};
+  for (const Out& o : outs) {
+    if (!o.dst) continue;
+    const size_t total = (size_t)n_pos * o.rows * d.M;
+    const size_t blocks = std::min<size_t>((total + 255) / 256, 148 * 64);
+    qmc::pack_kernel<T, T><<<(unsigned)blocks, 256, 0, stream>>>(o.dst, o.src, (size_t)n_pos, o.rows, d.M, 5 * ns, ns, 0);
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(QMC_ERR_CUDA, "kernel launch: %s (%s:%d)", cudaGetErrorString(e), __FILE__, __LINE__);
+  return QMC_OK;
+}
+
+}  // namespace
+
+extern "C" int qmc_spo_vgl_static(int32_t n_orb, const int32_t* grid, const double* box, int32_t coef_dtype,
+                                  const void* coefs_dev, int64_t orb_stride, int32_t n_pos, const double* r_dev,
+                                  void* phi, void* dphi, void* d2phi, void* stream)
+{
+  using namespace qmc;
+  if (!grid || !box) return fail(QMC_ERR_INVALID_ARG, "grid / box is NULL");
+  if (n_orb < 1) return fail(QMC_ERR_INVALID_ARG, "n_orb must be >= 1");
+  if (coef_dtype != 0 && coef_dtype != 1) return fail(QMC_ERR_INVALID_ARG, "coef_dtype must be 0 or 1");
+  const int vw = coef_dtype ? 2 : 4;
+  if (orb_stride < n_orb || orb_stride % vw) return fail(QMC_ERR_INVALID_ARG, "orb_stride must be >= n_orb and a multiple of %d", vw);
+  double tab = (double)orb_stride / vw;
+  for (int c = 0; c < 3; ++c) {
+    if (grid[c] < 1) return fail(QMC_ERR_INVALID_ARG, "grid must be >= 1");
+    if (!(box[c] > 0.0) || !std::isfinite(box[c])) return fail(QMC_ERR_INVALID_ARG, "box must be positive");
+    tab *= grid[c];
+  }
+  if (tab >= 4294967296.0) return fail(QMC_ERR_INVALID_ARG, "coefficient table larger than 2^32 16-byte vectors");
+  if (n_pos < 0) return fail(QMC_ERR_INVALID_ARG, "n_pos must be >= 0");
+  if (n_pos == 0) return QMC_OK;
+  if (!coefs_dev || !r_dev) return fail(QMC_ERR_INVALID_ARG, "coefs_dev / r_dev is NULL");
+  const size_t ns = align_up((size_t)n_orb, 16), elem = coef_dtype ? 8 : 4;
+  const size_t need = (size_t)n_pos * 5 * ns * elem;
+  if (need > (size_t)QMC_STATIC_SCRATCH_BYTES)
+    return fail(QMC_ERR_WORKSPACE, "qmc_spo_vgl_static: %d positions x %d orbitals need %zu bytes of scratch, the static array holds %zu "
+                "(at most %zu positions per call for this table)", n_pos, n_orb, need, (size_t)QMC_STATIC_SCRATCH_BYTES,
+                (size_t)QMC_STATIC_SCRATCH_BYTES / (5 * ns * elem));
+  void* scratch = nullptr;
+  int st = static_scratch_address(&scratch);
+  if (st) return st;
+  CrowdDev d;
+  memset(&d, 0, sizeof(d));
+  d.W = n_pos; d.M = n_orb; d.n = n_orb; d.N = 2 * n_orb; d.ns = (int)ns;
+  for (int a = 0; a < 3; ++a) {
+    d.grid[a] = grid[a];
+    d.box[a] = box[a];
+    d.inv_box[a] = 1.0 / box[a];
+    d.inv_h[a] = (double)grid[a] / box[a];
+    d.inv_grid[a] = 1.0 / (double)grid[a];
+  }
+  d.orb_stride_v = (unsigned)(orb_stride / vw);
+  d.tab_vecs = d.orb_stride_v;
+  d.coefs = coefs_dev;
+  cudaStream_t s = (cudaStream_t)stream;
+  return coef_dtype ? spo_vgl_static_t<double>(d, n_pos, r_dev, (double*)scratch, (double*)phi, (double*)dphi, (double*)d2phi, s)
+                    : spo_vgl_static_t<float>(d, n_pos, r_dev, (float*)scratch, (float*)phi, (float*)dphi, (float*)d2phi, s);
+}
