@@ -352,11 +352,27 @@ int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
   return QMC_OK;
 }
 
+// The strip kernel of a flush (section L0 of the window, -1 = all of it): 32-row strips where the shape allows them
+template <int KB, int L0, typename TB>
+void launch_strip(const CrowdDev& d, int spin, int wn, cudaStream_t st)
+{
+  // (fp32-stored inverses keep the 16-row kernel: with the conversions next to 254 registers the 32-row form was slower,
+  // 3.70 against 3.5 ms per flush at cfg 5, W = 4096)
+  if constexpr (KB >= 2 && sizeof(TB) == 8) {
+    if (d.ns % 32 == 0) {
+      dim3 grid32((d.ns + FLUSH32_NT - 1) / FLUSH32_NT, wn);
+      flush32_kernel<KB, L0, TB><<<grid32, FLUSH32_NT, 0, st>>>(d, spin);
+      return;
+    }
+  }
+  const int rows_per_cta = (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP;
+  dim3 grid((d.ns + rows_per_cta - 1) / rows_per_cta, wn);
+  flush_kernel<KB, L0, TB><<<grid, FLUSH_NT, 0, st>>>(d, spin);
+}
+
 template <int KDP>
 void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cudaStream_t st)
 {
-  const int rows_per_cta = (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP;
-  dim3 grid((d.ns + rows_per_cta - 1) / rows_per_cta, wn);
   if (from_window && KDP > 32) {
     // Two sections of 32 moves, each a complete flush applied to the result of the one before: the sequential
     // Sherman-Morrison updates B_{l+1} = B_l - (B_l phi_l - e_l) c_l^T compose section by section (c_l is the current
@@ -364,9 +380,9 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     // with four window blocks keeps its double-buffered operands in registers (eight spill or lose the double
     // buffer): 11.1 -> 7.7 ms per flush of 64 moves at cfg 5, W = 4096.
     flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)(1 + FINTRI_NT / 32) * 32 * 33 * 8, st>>>(d, 0);
-    flush_kernel<4, 0><<<grid, FLUSH_NT, 0, st>>>(d, spin);
+    launch_strip<4, 0, double>(d, spin, wn, st);
     flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)(1 + FINTRI_NT / 32) * 32 * 33 * 8, st>>>(d, 32);
-    flush_kernel<4, 32><<<grid, FLUSH_NT, 0, st>>>(d, spin);
+    launch_strip<4, 32, double>(d, spin, wn, st);
     return;
   }
   if (from_window) {
@@ -376,8 +392,14 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     dim3 fgrid((d.ns + fcols - 1) / fcols, wn);
     flush_finalize_kernel<KDP><<<fgrid, FINALIZE_NT, (size_t)KDP * KDP * 8, st>>>(d, spin);
   }
-  if (d.Binv32) flush_kernel<KDP / 8, -1, float><<<grid, FLUSH_NT, 0, st>>>(d, spin);   // D:R6, delay_rank <= 32: one pass
-  else flush_kernel<KDP / 8><<<grid, FLUSH_NT, 0, st>>>(d, spin);
+  if constexpr (KDP <= 32) {
+    if (d.Binv32) {   // D:R6, delay_rank <= 32: one pass, one rounding
+      launch_strip<KDP / 8, -1, float>(d, spin, wn, st);
+      return;
+    }
+  }
+  if constexpr (KDP <= 32) launch_strip<KDP / 8, -1, double>(d, spin, wn, st);
+  else flush_kernel<KDP / 8><<<dim3((d.ns + (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP - 1) / ((FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP), wn), FLUSH_NT, 0, st>>>(d, spin);
 }
 
 // Flush of walkers [w0, w0 + wn) on stream st (the whole crowd on the crowd's stream by default).

@@ -567,4 +567,157 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
   }
 }
 
+// ---- 32-row strips: four 8-row blocks per warp, so every V / Z fragment set feeds twice the DMMAs of the 16-row kernel
+// above (64 per set at KB = 4), fragment sets double-buffered in registers (254 registers, two CTAs of four warps per
+// SM).  Measured at cfg 5, W = 4096, k = 32 (B200, round 2): 2.96 ms per launch against 3.13 ms, DMMA pipe 70 % busy
+// against 67 % (GEMM 2 sums the window blocks in one chain per tile instead of two: rounding-level differences).  The larger strips in flight
+// (98 KB per warp, 116 MB over the GPU) miss L2 more often on their second read: 13.2 GB of DRAM traffic against 12.2 GB
+// for 9.66 GB algorithmic -- the kernel is bound by the latency of its fragment loads next to the DMMAs, not by DRAM
+// bandwidth, so the trade pays.  Single-buffered at 168 registers (three CTAs per SM, 124 B spill) it ran at 3.6 ms,
+// single-buffered at 198 registers (two CTAs) at 4.1 ms; CTAs of one or two warps at the same occupancy: no change.
+// Used for fp64-stored inverses when ns % 32 == 0 and the window has at least two blocks (KB >= 2); the 16-row kernel
+// serves the rest.
+#ifndef QMC_FLUSH32_MIN_CTAS
+#define QMC_FLUSH32_MIN_CTAS 2
+#endif
+#ifndef QMC_FLUSH32_NT
+#define QMC_FLUSH32_NT 128
+#endif
+constexpr int FLUSH32_NT = QMC_FLUSH32_NT;
+template <int KB>
+struct Frag1x4 {
+  double a[4][4], v[KB][4];
+};
+template <int KB, typename TB>
+__device__ __forceinline__ void load_frag1x4(Frag1x4<KB>& f, const TB* ap, const double* vp, int s, int ns, int m, int mb, int g)
+{
+#pragma unroll
+  for (int i = 0; i < 4; ++i) ld_b4(ap + (size_t)(8 * i) * ns + s, f.a[i]);
+#pragma unroll
+  for (int b = 0; b < KB; ++b) {
+    f.v[b][0] = f.v[b][1] = f.v[b][2] = f.v[b][3] = 0.0;
+    if (b < mb && 8 * b + g < m) ld32(vp + (size_t)(8 * b) * ns + s, f.v[b]);
+  }
+}
+template <int KB>
+__device__ __forceinline__ void mma_frag1x4(double (&acc)[4][KB][2], const Frag1x4<KB>& f, int mb)
+{
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+#pragma unroll
+    for (int b = 0; b < KB; ++b)
+      if (b < mb) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) dmma884(acc[i][b], f.a[i][q], f.v[b][q]);
+      }
+}
+template <int KB>
+struct Frag2x4 {
+  double x[4][4];
+  double2 z[KB][2];
+};
+template <int KB, typename TB>
+__device__ __forceinline__ void load_frag2x4(Frag2x4<KB>& f, const TB* ap, const double* zp, int j0, int ns, int m, int mb, int t)
+{
+#pragma unroll
+  for (int i = 0; i < 4; ++i) ld_b4(ap + (size_t)(8 * i) * ns + j0, f.x[i]);
+#pragma unroll
+  for (int b = 0; b < KB; ++b)
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      f.z[b][q] = make_double2(0.0, 0.0);
+      if (b < mb && 8 * b + 2 * t + q < m) f.z[b][q] = *reinterpret_cast<const double2*>(zp + (size_t)(8 * b + q) * ns + j0);
+    }
+}
+template <int KB, typename TB>
+__device__ __forceinline__ void mma_store_frag2x4(const Frag2x4<KB>& f, const double (&nw)[4][KB][2], int mb, TB* op, int ns)
+{
+  double de[4][2], dd[4][2];   // even / odd columns of the chunk: eight independent DMMA chains
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    de[i][0] = f.x[i][0]; de[i][1] = f.x[i][2];
+    dd[i][0] = f.x[i][1]; dd[i][1] = f.x[i][3];
+  }
+#pragma unroll
+  for (int q = 0; q < 2; ++q)
+#pragma unroll
+    for (int b = 0; b < KB; ++b)
+      if (b < mb) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          dmma884(de[i], nw[i][b][q], f.z[b][q].x);
+          dmma884(dd[i], nw[i][b][q], f.z[b][q].y);
+        }
+      }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) st_b4(op + (size_t)(8 * i) * ns, de[i][0], dd[i][0], de[i][1], dd[i][1]);
+}
+
+// L0, TB: as for flush_kernel.  grid = (ceil(ns / (32 warps per CTA)), W).
+template <int KB, int L0 = -1, typename TB = double>
+__global__ void __launch_bounds__(FLUSH32_NT, QMC_FLUSH32_MIN_CTAS) flush32_kernel(CrowdDev d, int spin)
+{
+  constexpr int l0 = L0 < 0 ? 0 : L0;
+  const int w = blockIdx.y + d.w0;
+  int m = d.mwin[w];
+  if constexpr (L0 < 0) {
+    if (m == 0) return;
+  } else {
+    m = min(m - l0, 8 * KB);
+    if (m <= 0) return;
+  }
+  const int ns = d.ns, kdp = d.kdp;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int row0 = (blockIdx.x * (FLUSH32_NT / 32) + warp) * 32;
+  if (row0 >= ns) return;
+  TB* B = carried_inverse<TB>(d) + ((size_t)w * 2 + spin) * ns * ns;
+  const int* rows = d.rows + (size_t)w * kdp + l0;
+  const int mb = (m + 7) >> 3;
+  TB* ap = B + (size_t)(row0 + g) * ns + 4 * t;
+  const double* vp = d.V + (size_t)w * kdp * ns + (size_t)(g + l0) * ns + 4 * t;
+  const double* zp = d.C + (size_t)w * kdp * ns + (size_t)(2 * t + l0) * ns + 2 * g;
+  double acc[4][KB][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int b = 0; b < KB; ++b) acc[i][b][0] = acc[i][b][1] = 0.0;
+  {
+    Frag1x4<KB> fa, fb;
+    load_frag1x4<KB>(fa, ap, vp, 0, ns, m, mb, g);
+    for (int s = 0; s < ns; s += 32) {
+      if (s + 16 < ns) load_frag1x4<KB>(fb, ap, vp, s + 16, ns, m, mb, g);
+      mma_frag1x4<KB>(acc, fa, mb);
+      if (s + 16 < ns) {
+        if (s + 32 < ns) load_frag1x4<KB>(fa, ap, vp, s + 32, ns, m, mb, g);
+        mma_frag1x4<KB>(acc, fb, mb);
+      }
+    }
+  }
+#pragma unroll
+  for (int b = 0; b < KB; ++b) {
+    if (b < mb) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int l = 8 * b + 2 * t + e;
+        const int rl = (l < m) ? rows[l] : -1;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[i][b][e] = (rl == row0 + 8 * i + g ? 1.0 : 0.0) - acc[i][b][e];
+      }
+    }
+  }
+  {
+    // chunks in reverse order: the strip lines GEMM 1 read last are the most likely to still be in L2
+    Frag2x4<KB> fa, fb;
+    load_frag2x4<KB>(fa, ap, zp, ns - 16, ns, m, mb, t);
+    for (int j0 = ns - 16; j0 >= 0; j0 -= 32) {
+      if (j0 >= 16) load_frag2x4<KB>(fb, ap, zp, j0 - 16, ns, m, mb, t);
+      mma_store_frag2x4<KB>(fa, acc, mb, ap + j0, ns);
+      if (j0 >= 16) {
+        if (j0 >= 32) load_frag2x4<KB>(fa, ap, zp, j0 - 32, ns, m, mb, t);
+        mma_store_frag2x4<KB>(fb, acc, mb, ap + j0 - 16, ns);
+      }
+    }
+  }
+}
+
 }  // namespace qmc
