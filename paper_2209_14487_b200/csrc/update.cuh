@@ -584,6 +584,12 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
 #define QMC_FLUSH32_NT 128
 #endif
 constexpr int FLUSH32_NT = QMC_FLUSH32_NT;
+// Window move held at position p of an 8-wide MMA tile.  The accumulator layout of GEMM 1 gives a lane the tile positions
+// 2 t and 2 t + 1, and GEMM 2 contracts over them in k-steps (b, q) = positions {2 t + q}: with position p holding move
+// 4 (p & 1) + (p >> 1) a k-step covers the four CONSECUTIVE moves 8 b + 4 q .. + 3, so the k-steps of the window's padding
+// can be left out in units of four moves instead of eight (m = 27 accepted moves of 32 on average at cfg 5).
+__device__ __forceinline__ int win_pos(int p) { return 4 * (p & 1) + (p >> 1); }
+
 template <int KB>
 struct Frag1x4 {
   double a[4][4], v[KB][4];
@@ -596,7 +602,7 @@ __device__ __forceinline__ void load_frag1x4(Frag1x4<KB>& f, const TB* ap, const
 #pragma unroll
   for (int b = 0; b < KB; ++b) {
     f.v[b][0] = f.v[b][1] = f.v[b][2] = f.v[b][3] = 0.0;
-    if (b < mb && 8 * b + g < m) ld32(vp + (size_t)(8 * b) * ns + s, f.v[b]);
+    if (b < mb && 8 * b + win_pos(g) < m) ld32(vp + (size_t)(8 * b) * ns + s, f.v[b]);
   }
 }
 template <int KB>
@@ -626,11 +632,11 @@ __device__ __forceinline__ void load_frag2x4(Frag2x4<KB>& f, const TB* ap, const
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
       f.z[b][q] = make_double2(0.0, 0.0);
-      if (b < mb && 8 * b + 2 * t + q < m) f.z[b][q] = *reinterpret_cast<const double2*>(zp + (size_t)(8 * b + q) * ns + j0);
+      if (8 * b + 4 * q + t < m) f.z[b][q] = *reinterpret_cast<const double2*>(zp + (size_t)(8 * b + 4 * q) * ns + j0);
     }
 }
 template <int KB, typename TB>
-__device__ __forceinline__ void mma_store_frag2x4(const Frag2x4<KB>& f, const double (&nw)[4][KB][2], int mb, TB* op, int ns)
+__device__ __forceinline__ void mma_store_frag2x4(const Frag2x4<KB>& f, const double (&nw)[4][KB][2], int m, TB* op, int ns)
 {
   double de[4][2], dd[4][2];   // even / odd columns of the chunk: eight independent DMMA chains
 #pragma unroll
@@ -639,16 +645,22 @@ __device__ __forceinline__ void mma_store_frag2x4(const Frag2x4<KB>& f, const do
     dd[i][0] = f.x[i][1]; dd[i][1] = f.x[i][3];
   }
 #pragma unroll
-  for (int q = 0; q < 2; ++q)
+  for (int b = 0; b < KB; ++b)
+    if (8 * b < m) {
+      // k-step (b, q) = window moves 8 b + 4 q .. + 3 (win_pos): the second one is skipped when none of them was accepted
 #pragma unroll
-    for (int b = 0; b < KB; ++b)
-      if (b < mb) {
+      for (int i = 0; i < 4; ++i) {
+        dmma884(de[i], nw[i][b][0], f.z[b][0].x);
+        dmma884(dd[i], nw[i][b][0], f.z[b][0].y);
+      }
+      if (8 * b + 4 < m) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          dmma884(de[i], nw[i][b][q], f.z[b][q].x);
-          dmma884(dd[i], nw[i][b][q], f.z[b][q].y);
+          dmma884(de[i], nw[i][b][1], f.z[b][1].x);
+          dmma884(dd[i], nw[i][b][1], f.z[b][1].y);
         }
       }
+    }
 #pragma unroll
   for (int i = 0; i < 4; ++i) st_b4(op + (size_t)(8 * i) * ns, de[i][0], dd[i][0], de[i][1], dd[i][1]);
 }
@@ -674,9 +686,9 @@ __global__ void __launch_bounds__(FLUSH32_NT, QMC_FLUSH32_MIN_CTAS) flush32_kern
   const int* rows = d.rows + (size_t)w * kdp + l0;
   const int mb = (m + 7) >> 3;
   TB* ap = B + (size_t)(row0 + g) * ns + 4 * t;
-  const double* vp = d.V + (size_t)w * kdp * ns + (size_t)(g + l0) * ns + 4 * t;
-  const double* zp = d.C + (size_t)w * kdp * ns + (size_t)(2 * t + l0) * ns + 2 * g;
-  double acc[4][KB][2];
+  const double* vp = d.V + (size_t)w * kdp * ns + (size_t)(win_pos(g) + l0) * ns + 4 * t;
+  const double* zp = d.C + (size_t)w * kdp * ns + (size_t)(t + l0) * ns + 2 * g;
+  double acc[4][KB][2];   // acc[i][b][e]: row 8 i + g of the strip, window move 8 b + win_pos(2 t + e) = 8 b + 4 e + t
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -698,7 +710,7 @@ __global__ void __launch_bounds__(FLUSH32_NT, QMC_FLUSH32_MIN_CTAS) flush32_kern
     if (b < mb) {
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
-        const int l = 8 * b + 2 * t + e;
+        const int l = 8 * b + 4 * e + t;
         const int rl = (l < m) ? rows[l] : -1;
 #pragma unroll
         for (int i = 0; i < 4; ++i) acc[i][b][e] = (rl == row0 + 8 * i + g ? 1.0 : 0.0) - acc[i][b][e];
@@ -711,10 +723,10 @@ __global__ void __launch_bounds__(FLUSH32_NT, QMC_FLUSH32_MIN_CTAS) flush32_kern
     load_frag2x4<KB>(fa, ap, zp, ns - 16, ns, m, mb, t);
     for (int j0 = ns - 16; j0 >= 0; j0 -= 32) {
       if (j0 >= 16) load_frag2x4<KB>(fb, ap, zp, j0 - 16, ns, m, mb, t);
-      mma_store_frag2x4<KB>(fa, acc, mb, ap + j0, ns);
+      mma_store_frag2x4<KB>(fa, acc, m, ap + j0, ns);
       if (j0 >= 16) {
         if (j0 >= 32) load_frag2x4<KB>(fa, ap, zp, j0 - 32, ns, m, mb, t);
-        mma_store_frag2x4<KB>(fb, acc, mb, ap + j0 - 16, ns);
+        mma_store_frag2x4<KB>(fb, acc, m, ap + j0 - 16, ns);
       }
     }
   }
