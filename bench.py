@@ -494,7 +494,13 @@ def run_cuda(args):
         kdp = 8
         while kdp < kd:
             kdp *= 2
-        executed = useful * (4 * n * n * kdp + 2 * n * kdp * kdp) / max(alg["flush"]["flops"] / W, 1.0)
+        # executed DMMA work: GEMM 1 pads the window to whole 8-move blocks (~ kdp); GEMM 2 of the 32-row strip kernel
+        # (fp64 inverses, n % 32 == 0, kdp >= 16) skips the k-steps of padding in units of four moves (~ m + 1.5 on average)
+        k2 = kdp
+        if n % 32 == 0 and kdp >= 16:   # the timed crowd carries fp64 inverses
+            acc_moves = (alg["flush"]["flops"] / W) / (4.0 * n * n)      # ~ accepted moves per flush (finalize term small)
+            k2 = min(float(kdp), acc_moves + 1.5)
+        executed = useful * (2 * n * n * kdp + 2 * n * n * k2 + 2 * n * kdp * kdp) / max(alg["flush"]["flops"] / W, 1.0)
         # denominator: whichever is larger of what cuBLAS DGEMM reaches in this run and the DMMA issue ceiling
         peak64 = max(probe or 0.0, FP64_DMMA_CEILING_TFLOPS)
         extra_rooflines["flush"] = with_traffic({

@@ -353,15 +353,19 @@ int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
 }
 
 // The strip kernel of a flush (section L0 of the window, -1 = all of it): 32-row strips where the shape allows them
+#ifndef QMC_FLUSH32_MIN_NS
+#define QMC_FLUSH32_MIN_NS 32
+#endif
 template <int KB, int L0, typename TB>
 void launch_strip(const CrowdDev& d, int spin, int wn, cudaStream_t st)
 {
   // (fp32-stored inverses keep the 16-row kernel: with the conversions next to 254 registers the 32-row form was slower,
   // 3.70 against 3.5 ms per flush at cfg 5, W = 4096)
   if constexpr (KB >= 2 && sizeof(TB) == 8) {
-    if (d.ns % 32 == 0) {
-      dim3 grid32((d.ns + FLUSH32_NT - 1) / FLUSH32_NT, wn);
-      flush32_kernel<KB, L0, TB><<<grid32, FLUSH32_NT, 0, st>>>(d, spin);
+    if (d.ns % 32 == 0 && d.ns >= QMC_FLUSH32_MIN_NS) {
+      const int nt = (d.ns / 32) % (FLUSH32_NT / 32) == 0 ? FLUSH32_NT : 32;
+      dim3 grid32((d.ns + nt - 1) / nt, wn);
+      flush32_kernel<KB, L0, TB><<<grid32, nt, 0, st>>>(d, spin);
       return;
     }
   }

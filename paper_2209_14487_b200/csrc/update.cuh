@@ -665,7 +665,9 @@ __device__ __forceinline__ void mma_store_frag2x4(const Frag2x4<KB>& f, const do
   for (int i = 0; i < 4; ++i) st_b4(op + (size_t)(8 * i) * ns, de[i][0], dd[i][0], de[i][1], dd[i][1]);
 }
 
-// L0, TB: as for flush_kernel.  grid = (ceil(ns / (32 warps per CTA)), W).
+// L0, TB: as for flush_kernel.  grid = (ceil(ns / (32 warps per CTA)), W); CTAs of four warps when the strips of a matrix fill
+// them, else of one warp (n = 192: 6 strips, n = 96: 3 -- half-empty CTAs hold registers for nothing: cfg 4 42.3 -> 44.3 M,
+// cfg 3 67.5 -> 70.3 M moves/s; at n = 384 one-warp CTAs are 0.25 % slower).
 template <int KB, int L0 = -1, typename TB = double>
 __global__ void __launch_bounds__(FLUSH32_NT, QMC_FLUSH32_MIN_CTAS) flush32_kernel(CrowdDev d, int spin)
 {
@@ -680,7 +682,7 @@ __global__ void __launch_bounds__(FLUSH32_NT, QMC_FLUSH32_MIN_CTAS) flush32_kern
   }
   const int ns = d.ns, kdp = d.kdp;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  const int row0 = (blockIdx.x * (FLUSH32_NT / 32) + warp) * 32;
+  const int row0 = (blockIdx.x * (blockDim.x >> 5) + warp) * 32;   // CTAs of FLUSH32_NT or of 32 threads (launch_strip)
   if (row0 >= ns) return;
   TB* B = carried_inverse<TB>(d) + ((size_t)w * 2 + spin) * ns * ns;
   const int* rows = d.rows + (size_t)w * kdp + l0;
