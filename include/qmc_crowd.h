@@ -225,6 +225,11 @@ int qmc_crowd_set_option(qmc_crowd_t* crowd, int option, int value);
  * sweep (counted on the crowd's sweep index, so the schedule does not depend on how sweeps are batched into calls);
  * 0 = never (default).                                                                                          */
 #define QMC_OPT_RECOMPUTE_EVERY 3
+/* option 4 (QMC_OPT_STRIP_ROWS): rows of the inverse a warp of the flush strip kernel owns: 0 = automatic (default: 32 for
+ * fp64-stored inverses with ns % 32 == 0, a delay rank >= 16 and a crowd of at least two waves of 32-row strips, else 16),
+ * 16 or 32 = forced where the shape allows it (32 needs ns % 32 == 0, fp64 storage and a delay rank >= 16; otherwise 16
+ * is used).  Both kernels compute the same update (rounding-level differences); tests force each one. */
+#define QMC_OPT_STRIP_ROWS 4
 
 /* kernel classes of the hot path, index into qmc_crowd_get_profile's arrays */
 enum {

@@ -18,6 +18,7 @@ QMC_OPT_GRAPH = 0
 QMC_OPT_PROFILE = 1
 QMC_OPT_SUBCROWDS = 2
 QMC_OPT_RECOMPUTE_EVERY = 3
+QMC_OPT_STRIP_ROWS = 4
 KERNEL_CLASSES = ("row_propose", "spline_vgl", "ratio_grad", "accept", "rank1", "flush", "ratio_accept",
                   "window", "kinetic", "branch")
 

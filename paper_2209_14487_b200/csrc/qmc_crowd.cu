@@ -71,6 +71,7 @@ struct qmc_crowd {
   uint32_t sweep_host;
   int use_graph;
   int n_sub;                        // sub-crowds of qmc_sweep (delay_rank > 1), each on its own stream; 0 = automatic
+  int strip_rows;                   // QMC_OPT_STRIP_ROWS: 0 = automatic, 16 / 32 = forced
   int recompute_every;              // qmc_sweep recomputes the inverses every this many sweeps (0 = never)
   int n_sm;                         // SMs of the device (sizes the automatic sub-crowd choice)
   cudaStream_t sub_stream[4];
@@ -353,16 +354,16 @@ int launch_accept_t(qmc_crowd* c, int k, unsigned char* acc_out)
 }
 
 // The strip kernel of a flush (section L0 of the window, -1 = all of it): 32-row strips where the shape allows them
-#ifndef QMC_FLUSH32_MIN_NS
-#define QMC_FLUSH32_MIN_NS 32
-#endif
 template <int KB, int L0, typename TB>
-void launch_strip(const CrowdDev& d, int spin, int wn, cudaStream_t st)
+void launch_strip(const CrowdDev& d, int spin, int wn, cudaStream_t st, int strip_rows)
 {
   // (fp32-stored inverses keep the 16-row kernel: with the conversions next to 254 registers the 32-row form was slower,
   // 3.70 against 3.5 ms per flush at cfg 5, W = 4096)
   if constexpr (KB >= 2 && sizeof(TB) == 8) {
-    if (d.ns % 32 == 0 && d.ns >= QMC_FLUSH32_MIN_NS) {
+    // small crowds keep 16-row strips: below ~2 waves of 32-row strip warps (8 per SM) the shorter chains of twice as many
+    // warps win (cfg 5, k = 32: W = 64 +1.4 %, W = 128 +4 %; from W = 256 on the 32-row kernel is faster)
+    const bool want32 = strip_rows ? strip_rows == 32 : (size_t)wn * (d.ns / 32) >= 2368;
+    if (d.ns % 32 == 0 && want32) {
       const int nt = (d.ns / 32) % (FLUSH32_NT / 32) == 0 ? FLUSH32_NT : 32;
       dim3 grid32((d.ns + nt - 1) / nt, wn);
       flush32_kernel<KB, L0, TB><<<grid32, nt, 0, st>>>(d, spin);
@@ -375,7 +376,7 @@ void launch_strip(const CrowdDev& d, int spin, int wn, cudaStream_t st)
 }
 
 template <int KDP>
-void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cudaStream_t st)
+void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cudaStream_t st, int strip_rows)
 {
   if (from_window && KDP > 32) {
     // Two sections of 32 moves, each a complete flush applied to the result of the one before: the sequential
@@ -384,9 +385,9 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
     // with four window blocks keeps its double-buffered operands in registers (eight spill or lose the double
     // buffer): 11.1 -> 7.7 ms per flush of 64 moves at cfg 5, W = 4096.
     flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)(1 + FINTRI_NT / 32) * 32 * 33 * 8, st>>>(d, 0);
-    launch_strip<4, 0, double>(d, spin, wn, st);
+    launch_strip<4, 0, double>(d, spin, wn, st, strip_rows);
     flush_finalize_tri_kernel<32><<<wn, FINTRI_NT, (size_t)(1 + FINTRI_NT / 32) * 32 * 33 * 8, st>>>(d, 32);
-    launch_strip<4, 32, double>(d, spin, wn, st);
+    launch_strip<4, 32, double>(d, spin, wn, st, strip_rows);
     return;
   }
   if (from_window) {
@@ -398,11 +399,11 @@ void launch_flush_kdp(const CrowdDev& d, int spin, bool from_window, int wn, cud
   }
   if constexpr (KDP <= 32) {
     if (d.Binv32) {   // D:R6, delay_rank <= 32: one pass, one rounding
-      launch_strip<KDP / 8, -1, float>(d, spin, wn, st);
+      launch_strip<KDP / 8, -1, float>(d, spin, wn, st, strip_rows);
       return;
     }
   }
-  if constexpr (KDP <= 32) launch_strip<KDP / 8, -1, double>(d, spin, wn, st);
+  if constexpr (KDP <= 32) launch_strip<KDP / 8, -1, double>(d, spin, wn, st, strip_rows);
   else flush_kernel<KDP / 8><<<dim3((d.ns + (FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP - 1) / ((FLUSH_NT / 32) * FLUSH_ROWS_PER_WARP), wn), FLUSH_NT, 0, st>>>(d, spin);
 }
 
@@ -414,10 +415,10 @@ int launch_flush(qmc_crowd* c, int spin, bool from_window = false, int w0 = 0, i
   d.w0 = w0;
   ProfScope ps(c, QMC_K_FLUSH);
   switch (d.kdp) {
-    case 8: launch_flush_kdp<8>(d, spin, from_window, wn, st); break;
-    case 16: launch_flush_kdp<16>(d, spin, from_window, wn, st); break;
-    case 32: launch_flush_kdp<32>(d, spin, from_window, wn, st); break;
-    case 64: launch_flush_kdp<64>(d, spin, from_window, wn, st); break;
+    case 8: launch_flush_kdp<8>(d, spin, from_window, wn, st, c->strip_rows); break;
+    case 16: launch_flush_kdp<16>(d, spin, from_window, wn, st, c->strip_rows); break;
+    case 32: launch_flush_kdp<32>(d, spin, from_window, wn, st, c->strip_rows); break;
+    case 64: launch_flush_kdp<64>(d, spin, from_window, wn, st, c->strip_rows); break;
     default: return fail(QMC_ERR_INVALID_ARG, "unsupported padded delay rank %d", d.kdp);
   }
   ++c->launches;
@@ -680,6 +681,7 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
   c->sweep_host = 0;
   c->use_graph = 1;
   c->n_sub = 0;
+  c->strip_rows = 0;
   c->recompute_every = 0;
   {
     int devid = 0;
@@ -1157,6 +1159,12 @@ int qmc_crowd_set_option(qmc_crowd_t* c, int option, int value)
   if (option == QMC_OPT_SUBCROWDS) {
     if (value < 0 || value > 4) return fail(QMC_ERR_INVALID_ARG, "sub-crowds must be in [0,4] (0 = automatic)");
     c->n_sub = value;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    return QMC_OK;
+  }
+  if (option == QMC_OPT_STRIP_ROWS) {
+    if (value != 0 && value != 16 && value != 32) return fail(QMC_ERR_INVALID_ARG, "strip rows must be 0 (automatic), 16 or 32");
+    c->strip_rows = value;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     return QMC_OK;
   }

@@ -24,10 +24,12 @@ from gpu_util import FreeRunningCheck, make_pair, npy, relerr, straddled_walkers
 
 pytestmark = pytest.mark.gpu
 
-def _free_running_vs_oracle(wl, sweeps):
+def _free_running_vs_oracle(wl, sweeps, options=()):
     """qmc_sweep against the oracle's crowd, sweep by sweep, by the P-free protocol with classification
     (gpu_util.FreeRunningCheck): bit-exact up to a rounding straddle the oracle itself reports as undecided."""
     crowd, osys, _, pos = make_pair(wl)
+    for opt, val in options:
+        crowd.set_option(opt, val)
     oc = oracle.OracleCrowd(osys, pos)
     chk = FreeRunningCheck(wl.n_walkers, wl.tau)
     Rg_prev, Ro_prev = pos, pos
@@ -143,6 +145,58 @@ def test_sweep_equals_step_calls_in_the_benched_window_class(n_elec, kd, sweeps)
             assert not off.any() or relerr(Ba[off], Bb[off]) < 1e-5
         R_prev = Ra
     assert a.stats() == b.stats()
+
+
+# name: (n_elec, grid, W, delay_rank, sweeps): shapes of the 32-row strip kernel (ns % 32 == 0, delay rank >= 16)
+STRIP_CASES = {
+    "n96_k32_three_strips_one_warp_ctas": (192, 8, 5, 32, 1),
+    "n128_k32_four_strips_one_cta": (256, 8, 3, 32, 1),
+    "n192_k16_two_window_blocks": (384, 9, 3, 16, 1),
+    "n128_k64_two_sections": (256, 8, 3, 64, 1),
+    "n384_k32_benched_instance": (768, 9, 3, 32, 1),
+}
+
+
+@pytest.mark.parametrize("rows", [32, 16])
+@pytest.mark.parametrize("name", list(STRIP_CASES))
+def test_both_strip_kernels_of_the_flush_match_the_oracle(name, rows):
+    """QMC_OPT_STRIP_ROWS: flush32_kernel (32-row strips, window moves permuted inside the MMA tiles, padding k-steps
+    skipped; what crowds of two waves and more run at cfgs 3-5) and flush_kernel (16-row strips; small crowds, fp32-stored
+    inverses) forced in turn on crowds of a few walkers: qmc_sweep against the oracle's C6 flush, positions bit for bit
+    up to a classified rounding straddle, inverses 1e-10; then the step-call flush (qmc_flush_delayed, the C / S^-T form
+    of the finalize) of a teacher-forced window against oracle.delayed_flush."""
+    import paper_2209_14487_b200 as q
+    n_elec, grid, W, kd, sweeps = STRIP_CASES[name]
+    wl = qi.small_workload(n_elec=n_elec, grid=grid, box=0.9 * n_elec ** (1 / 3), coef_dtype="f64", coef_dist="uniform",
+                           n_walkers=W, tau=0.02, delay_rank=kd, cfg=37)
+    crowd, chk = _free_running_vs_oracle(wl, sweeps, options=[(q.QMC_OPT_STRIP_ROWS, rows)])
+    assert chk.exact_moves >= 0.2 * W * n_elec * sweeps
+    # step calls: one window of the up spin, flushed by qmc_flush_delayed with the same kernel forced
+    crowd.set_sweep_index(sweeps)
+    B0 = npy(crowd.inverse(0))
+    for k in range(min(kd, n_elec // 2)):
+        crowd.qmc_spo_vgl(k)
+        crowd.qmc_ratio_grad(k)
+        crowd.qmc_accept_reject(k)
+    m, rws, V, Cm, _ = (npy(x) for x in crowd.window())
+    crowd.qmc_flush_delayed()
+    B1 = npy(crowd.inverse(0))
+    assert m.sum() > 0
+    for w in range(W):
+        mw = int(m[w])
+        ref = oracle.delayed_flush(B0[w], rws[w, :mw], V[w, :mw], Cm[w, :mw]) if mw else B0[w]
+        assert relerr(B1[w], ref) < 1e-10
+
+
+def test_strip_rows_option_is_validated():
+    import paper_2209_14487_b200 as q
+    wl = qi.small_workload(n_elec=16, grid=8, box=4.0, coef_dtype="f64", n_walkers=2, delay_rank=4, cfg=38)
+    crowd, _, _, _ = make_pair(wl)
+    with pytest.raises(q.QmcError) as e:
+        crowd.set_option(q.QMC_OPT_STRIP_ROWS, 8)
+    assert e.value.status == q.QMC_ERR_INVALID_ARG
+    crowd.set_option(q.QMC_OPT_STRIP_ROWS, 32)      # n = 8: the shape does not allow 32-row strips, 16 are used
+    crowd.qmc_sweep(1)
 
 
 # ---- several crowds / sub-crowds against ONE oracle crowd (fp64 tables) ----------------------------------------
