@@ -574,7 +574,14 @@ __global__ void __launch_bounds__(FLUSH_NT, QMC_FLUSH_MIN_CTAS) flush_kernel(Cro
 // (98 KB per warp, 116 MB over the GPU) miss L2 more often on their second read: 13.2 GB of DRAM traffic against 12.2 GB
 // for 9.66 GB algorithmic -- the kernel is bound by the latency of its fragment loads next to the DMMAs, not by DRAM
 // bandwidth, so the trade pays.  Single-buffered at 168 registers (three CTAs per SM, 124 B spill) it ran at 3.6 ms,
-// single-buffered at 198 registers (two CTAs) at 4.1 ms; CTAs of one or two warps at the same occupancy: no change.
+// single-buffered at 198 registers (two CTAs) at 4.1 ms; CTAs of one or two warps at the same occupancy: no change;
+// prefetch.global.L2 of the strip 4 or 8 chunks ahead of the fragment loads (both GEMMs): 3.45 ms against 3.31 ms per
+// flush; the first 3 or 6 chunks of every strip (the ones least likely to survive in L2 until GEMM 2 comes back to them)
+// kept in otherwise unused shared memory between the two GEMMs, conflict-free 16-byte pieces: 3.70 ms against 3.37 ms
+// (shared-memory traffic next to the DMMAs costs more than the DRAM re-reads it saves, as with round 1's operand ring).
+// With 4 KB of strip per warp in flight (8 warps per SM, ~1 us of loaded DRAM latency) the kernel moves 4.5 TB/s of mixed
+// read / write traffic (0.69 of the copy rate) next to a DMMA pipe that is 68 % busy: both are near what this structure
+// can feed; the overfetch of the second strip read (3.6 of its 4.8 GB miss L2) is what is left to remove.
 // Used for fp64-stored inverses when ns % 32 == 0 and the window has at least two blocks (KB >= 2); the 16-row kernel
 // serves the rest.
 #ifndef QMC_FLUSH32_MIN_CTAS
