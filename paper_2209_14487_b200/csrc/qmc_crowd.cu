@@ -72,6 +72,7 @@ struct qmc_crowd {
   int use_graph;
   int n_sub;                        // sub-crowds of qmc_sweep (delay_rank > 1), each on its own stream; 0 = automatic
   int strip_rows;                   // QMC_OPT_STRIP_ROWS: 0 = automatic, 16 / 32 = forced
+  int smem_optin;                   // cudaDevAttrMaxSharedMemoryPerBlockOptin of the device
   int recompute_every;              // qmc_sweep recomputes the inverses every this many sweeps (0 = never)
   int n_sm;                         // SMs of the device (sizes the automatic sub-crowd choice)
   cudaStream_t sub_stream[4];
@@ -477,6 +478,9 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   // shape-specialised instances for the BASELINE.json shapes with n a multiple of 16 (cfgs 3, 4, 5): see window.cuh
   const bool shape_ok = sizeof(T) == 4 && d.n == d.ns && d.M == d.n && d.tab_vecs >= (unsigned)d.ns / 4;
   const bool spec = nt == 128 && shape_ok;
+  // 512-thread class (one walker per SM): the block rows in shared memory when they fit next to the move's own state
+  const size_t smem_sb = smem + (size_t)d.kdp * d.ns * 8;
+  const bool sb_ok = smem_sb + 1024 <= (size_t)c->smem_optin;
   if (d.Binv32) {   // mixed precision (D:R6): the block's B0 rows are fp32
     if (spec && d.ns == 384) window_kernel<T, 128, 384, float><<<wn, 128, smem, st>>>(d, k0, cnt);
     else if (nt == 512) window_kernel<T, 512, 0, float><<<wn, 512, smem, st>>>(d, k0, cnt);
@@ -486,9 +490,13 @@ int launch_window_t(qmc_crowd* c, int k0, int cnt, int w0, int wn, cudaStream_t 
   else if (spec && d.ns == 192) window_kernel<T, 128, 192><<<wn, 128, smem, st>>>(d, k0, cnt);
   else if (spec && d.ns == 96) window_kernel<T, 128, 96><<<wn, 128, smem, st>>>(d, k0, cnt);
   else if (shape_ok && d.ns == 384 && nt == 256) window_kernel<T, 256, 384><<<wn, 256, smem, st>>>(d, k0, cnt);   // small crowds of cfg 5
+  else if (shape_ok && d.ns == 384 && nt == 512 && sb_ok) window_kernel<T, 512, 384, double, true><<<wn, 512, smem_sb, st>>>(d, k0, cnt);
   else if (shape_ok && d.ns == 384 && nt == 512) window_kernel<T, 512, 384><<<wn, 512, smem, st>>>(d, k0, cnt);
   else switch (nt) {   // the class of the WHOLE crowd: a split into sub-crowds never changes a reduction tree
-    case 512: window_kernel<T, 512><<<wn, 512, smem, st>>>(d, k0, cnt); break;
+    case 512:
+      if (sb_ok) window_kernel<T, 512, 0, double, true><<<wn, 512, smem_sb, st>>>(d, k0, cnt);
+      else window_kernel<T, 512><<<wn, 512, smem, st>>>(d, k0, cnt);
+      break;
     case 256: window_kernel<T, 256><<<wn, 256, smem, st>>>(d, k0, cnt); break;
     default: window_kernel<T, 128><<<wn, 128, smem, st>>>(d, k0, cnt); break;
   }
@@ -518,6 +526,7 @@ cudaError_t raise_smem_limits_t(int optin)
                        (const void*)window_kernel<T, 128, 0, float>, (const void*)window_kernel<T, 256, 0, float>,
                        (const void*)window_kernel<T, 512, 0, float>,
                        (const void*)window_kernel<T, 256>, (const void*)window_kernel<T, 512>,
+                       (const void*)window_kernel<T, 512, 384, double, true>, (const void*)window_kernel<T, 512, 0, double, true>,
                        (const void*)sweep1_kernel<T>, (const void*)spline_build_kernel<T>, (const void*)spline_build_cells_kernel<T>,
                        (const void*)kinetic_kernel<T>};
   for (const void* f : fns) {
@@ -687,6 +696,8 @@ int qmc_crowd_create(const qmc_crowd_desc* desc, const double* pos_dev, qmc_crow
     int devid = 0;
     c->n_sm = 148;
     if (cudaGetDevice(&devid) == cudaSuccess) cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, devid);
+    c->smem_optin = 48 * 1024;
+    if (cudaGetDevice(&devid) == cudaSuccess) cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, devid);
   }
   for (int i = 0; i < 4; ++i) { c->sub_stream[i] = nullptr; c->ev_join[i] = nullptr; }
   c->ev_fork = nullptr;

@@ -290,9 +290,13 @@ __device__ __forceinline__ void block_rows_update(const TS* src, double* dst, in
 // instruction stream, a third of which was integer / control overhead (ncu r2).  NS = 0: any shape.
 // TB: storage type of the carried inverse (double; float = mixed precision, D:R6: the block's B0 rows are widened
 // on load; everything the window itself writes -- Bcur, V, Cp -- stays fp64).
-template <typename T, int NT, int NS = 0, typename TB = double>
+// SB: the window's block of inverse rows (kdp x ns doubles, 98 KB at cfg 5) lives in shared memory instead of the d.C
+// buffer -- for the 512-thread class (crowds of at most one walker per SM), where a move is a latency chain and the block-row
+// update of an accepted move otherwise waits on L2 round trips; dynamic smem: win_layout(...).total + kdp ns doubles.
+template <typename T, int NT, int NS = 0, typename TB = double, bool SB = false>
 __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) window_kernel(CrowdDev d, int k0, int cnt)
 {
+  static_assert(!SB || sizeof(TB) == 8, "the shared-memory block is loaded by plain copies of fp64 rows");
   extern __shared__ double sm[];
   __shared__ SplineW<T> sw;
   const int w = blockIdx.x + d.w0, ns = sh_ns<NS>(d), nN = sh_N<NS>(d), kdp = d.kdp, tid = threadIdx.x;
@@ -312,7 +316,7 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
   const int spin = k0 / sh_n<NS>(d), kk0 = k0 - spin * sh_n<NS>(d);
   const TB* blk = carried_inverse<TB>(d) + (((size_t)w * 2 + spin) * ns + kk0) * ns;  // B0 rows of the window
   constexpr bool B64 = sizeof(TB) == 8;
-  double* Bcur = d.C + (size_t)w * kdp * ns;                              // their current values, once m > 0
+  double* Bcur = SB ? sm + L.total : d.C + (size_t)w * kdp * ns;          // their current values, once m > 0 (SB: always)
   double* Cp = d.Cp + (size_t)w * kdp * ns;
   double* V = d.V + (size_t)w * kdp * ns;
   double* Rg = d.R + (size_t)w * nN * 3;
@@ -327,8 +331,12 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
   cp_async_cta<NT>(cbuf, cache0, cache_bytes);
   for (int j = tid; j < 3 * nN; j += NT) R_s[j] = Rg[j];
   if (tid >= 32 && tid < 36) gauss_pieces(d, w, k0, tid - 32, gauss);
-  for (int j = tid; j < (cnt - 1) * ns * (int)sizeof(TB) / 128; j += NT)
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
+  if constexpr (SB) {
+    cp_async_cta<NT>(Bcur, blk, cnt * row_bytes);
+  } else {
+    for (int j = tid; j < (cnt - 1) * ns * (int)sizeof(TB) / 128; j += NT)
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(blk + ns) + (size_t)j * 128));
+  }
   cp_async_wait_all();
   __syncthreads();
   J2Part jnext;   // Jastrow partial of the coming move's electron at its current position
@@ -359,6 +367,17 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
     win_gold_propose<T, NT, NS>(d, k, b_s, ccur, R_s, jnext, i ? pairk + 4 * prev_acc : nullptr, ms, red, gauss, &sw);
     __syncthreads();   // r' and the spline weights of r' are visible
     PH(1);
+    if constexpr (NT >= 256) {
+      // small crowds (a move is a latency chain): the 64 stencil rows of r' are pulled into L2 under the Jastrow sums, so
+      // that the gather below waits for L2 instead of DRAM.  (At full crowds the same prefetch bought nothing: DESIGN 6.)
+      const char* tab = static_cast<const char*>(d.coefs);
+      const int lpr = (int)((min((unsigned)ns / Vec16<T>::W, d.tab_vecs) + 7) / 8);   // 128-byte lines of a row that hold orbitals
+      for (int j = tid; j < 64 * lpr; j += NT) {
+        const int row = j / lpr, l = j - row * lpr;
+        const unsigned base = sw.off[0][row >> 4] + sw.off[1][(row >> 2) & 3] + sw.off[2][row & 3];
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(tab + (size_t)base * 16 + (size_t)l * 128));
+      }
+    }
     // ---- both Jastrow sums (at r' for the ratio, at r_{k+1} for the next proposal), four pair chains in flight ----
     J2Part jr;
     const double rn[3] = {ms.rn[0], ms.rn[1], ms.rn[2]};
@@ -391,7 +410,10 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
         }
       }
       if (warp == 3 % (NT / 32)) {
-        if (B64 || m) cp_async_warp(bn_s, (m ? Bcur : reinterpret_cast<const double*>(blk)) + (size_t)(i + 1) * ns, row_bytes);
+        if constexpr (SB) {
+          const double2* src = reinterpret_cast<const double2*>(Bcur + (size_t)(i + 1) * ns);
+          for (int j = lane; j < ns / 2; j += 32) reinterpret_cast<double2*>(bn_s)[j] = src[j];
+        } else if (B64 || m) cp_async_warp(bn_s, (m ? Bcur : reinterpret_cast<const double*>(blk)) + (size_t)(i + 1) * ns, row_bytes);
         else
           for (int j = lane; j < ns; j += 32) bn_s[j] = (double)blk[(size_t)(i + 1) * ns + j];
         cp_async_warp(cbuf + ((i + 1) & 1) * cstride, cache_g + 4 * ns, cache_bytes);
@@ -418,7 +440,8 @@ __global__ void __launch_bounds__(NT, NT == 128 ? QMC_WIN_MINCTAS : 512 / NT) wi
       if (tid == 0) rows_s[m] = kk0 + i;
       cp_async_wait_all();   // the stale copy of the next row has landed before the update overwrites it
       __syncthreads();
-      if constexpr (B64) block_rows_update<T, NT>(m ? Bcur : reinterpret_cast<const double*>(blk), Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
+      if constexpr (SB) block_rows_update<T, NT>(Bcur, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
+      else if constexpr (B64) block_rows_update<T, NT>(m ? Bcur : reinterpret_cast<const double*>(blk), Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
       else if (m) block_rows_update<T, NT>(Bcur, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
       else block_rows_update<T, NT, TB>(blk, Bcur, ns, i + 1, cnt, vgl_s, b_s, bn_s);
       ++m;
