@@ -116,12 +116,15 @@ def test_rank1_large_n_step_parity(n_elec, kd):
     assert n_acc > 0
 
 
-@pytest.mark.parametrize("n_elec,kd,sweeps", [(48, 8, 2), (192, 32, 1)])
-def test_sweep_equals_step_calls_in_the_benched_window_class(n_elec, kd, sweeps):
+@pytest.mark.parametrize("n_elec,kd,sweeps,W,box", [(48, 8, 2, 300, 6.0), (192, 32, 1, 300, 6.0), (768, 32, 1, 5, 8.2),
+                                                    (768, 32, 1, 160, 8.2)])
+def test_sweep_equals_step_calls_in_the_benched_window_class(n_elec, kd, sweeps, W, box):
     """qmc_sweep through window_kernel<float,128> (W = 300, fp32 table) against the three step calls, which
     test_gpu_step_parity compares with the oracle call by call: identical positions and decisions, inverses 1e-10.
-    n = 24: the generic instance; n = 96: a shape-specialised instance (window_kernel<float,128,96>, as cfgs 3-5 run)."""
-    wl = qi.small_workload(n_elec=n_elec, grid=10, box=6.0, coef_dtype="f32", coef_dist="normal", n_walkers=300,
+    n = 24: the generic instance; n = 96: a shape-specialised instance (window_kernel<float,128,96>, as cfgs 3-5 run);
+    n = 384 with 5 / 160 walkers: the small-crowd instances of cfg 5, window_kernel<float,512,384> with the block rows in
+    shared memory and window_kernel<float,256,384>."""
+    wl = qi.small_workload(n_elec=n_elec, grid=10, box=box, coef_dtype="f32", coef_dist="normal", n_walkers=W,
                            tau=0.02, delay_rank=kd, cfg=36)
     a, _, _, R_prev = make_pair(wl)
     b, _, _, _ = make_pair(wl)
@@ -137,12 +140,13 @@ def test_sweep_equals_step_calls_in_the_benched_window_class(n_elec, kd, sweeps)
             if (kk + 1) % kd == 0 or kk == n - 1:
                 b.qmc_flush_delayed()
         Ra, Rb = npy(a.positions()), npy(b.positions())
-        off = straddled_walkers(Ra, Rb, R_prev)
+        off = straddled_walkers(Ra, Rb, R_prev, cascade=n_elec >= 768)
         assert not off.any() or sweeps == 1   # a straddled walker is not followed into another sweep
         for spin in (0, 1):
             Ba, Bb = npy(a.inverse(spin)), npy(b.inverse(spin))
             assert relerr(Ba[~off], Bb[~off]) < 1e-10
-            assert not off.any() or relerr(Ba[off], Bb[off]) < 1e-5
+            # (departed walkers: positions within 1e-5 after up to 700 more moves, amplified by the matrices' conditioning)
+            assert not off.any() or relerr(Ba[off], Bb[off]) < (1e-3 if n_elec >= 768 else 1e-5)
         R_prev = Ra
     assert a.stats() == b.stats()
 
