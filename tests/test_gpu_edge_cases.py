@@ -85,17 +85,24 @@ def test_argument_and_state_errors():
     assert e.value.status == q.QMC_ERR_INVALID_ARG
 
 
-@pytest.mark.parametrize("tau,kd", [(1e-6, 8), (1e-6, 1), (0.6, 8), (0.6, 1), (0.6, 32)])
-def test_acceptance_extremes(tau, kd):
+@pytest.mark.parametrize("tau,kd,n_elec,rows", [(1e-6, 8, 80, 0), (1e-6, 1, 80, 0), (0.6, 8, 80, 0), (0.6, 1, 80, 0),
+                                                 (0.6, 32, 80, 0), (1e-6, 32, 128, 32), (0.6, 32, 128, 32),
+                                                 (0.6, 16, 128, 32), (0.6, 64, 256, 32)])
+def test_acceptance_extremes(tau, kd, n_elec, rows):
     """Nearly every move accepted (full windows, m = k) and nearly every move rejected (windows with m = 0 or 1, flushes
-    that have nothing to do): the free-running trajectory still equals the oracle's on an fp64 table."""
-    wl = qi.small_workload(n_elec=80, grid=12, box=7.0, coef_dtype="f64", coef_dist="uniform", n_walkers=5, tau=tau,
-                           delay_rank=kd, cfg=76)
+    that have nothing to do): the free-running trajectory still equals the oracle's on an fp64 table.  rows = 32: the
+    32-row strip kernel forced (QMC_OPT_STRIP_ROWS), whose GEMM 2 skips k-steps by the number of accepted moves -- windows
+    with m = 0, 1..4, 5..8 and full ones all occur."""
+    import paper_2209_14487_b200 as q
+    wl = qi.small_workload(n_elec=n_elec, grid=12, box=7.0 * (n_elec / 80) ** (1 / 3), coef_dtype="f64", coef_dist="uniform",
+                           n_walkers=5, tau=tau, delay_rank=kd, cfg=76)
     crowd, osys, _, pos = make_pair(wl)
+    if rows:
+        crowd.set_option(q.QMC_OPT_STRIP_ROWS, rows)
     oc = oracle.OracleCrowd(osys, pos)
     acc = oc.sweep(2)
     crowd.qmc_sweep(2)
-    frac = acc / (2 * 5 * 80)
+    frac = acc / (2 * 5 * n_elec)
     assert frac > 0.98 if tau < 1e-3 else frac < 0.5, frac
     assert crowd.stats()["accepted"] == acc
     assert np.array_equal(npy(crowd.positions()), oc.positions())
