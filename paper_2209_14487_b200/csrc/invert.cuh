@@ -159,14 +159,13 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
     __syncthreads();
     IPH(0);
     // The panel itself is eliminated in sub-panels of INVB_SB columns, the same right-looking scheme one level down:
-    // a pivot step touches n x SB elements (a warp takes four rows at a time, lane = (row, sub-panel column), the
+    // a pivot step touches n x SB elements (a warp takes sixteen rows at a time, lane = (row group, column pair), the
     // multiplier of a row is a shuffle, the row interchange is done on register copies of rows c and p, the search
     // for the next pivot rides on the update), and after each sub-panel the other 32 - SB panel columns get its row
     // swaps and one rank-SB update.  (Eliminating all 32 columns at every pivot step cost 67 of the kernel's 139 ms at
     // cfg 5, W = 4096.)
-    constexpr int NW = INVB2_NT / 32, SB = INVB_SB, RPW = 32 / SB;   // RPW rows per warp pass
-    static_assert(INVB_NB == 32 && SB == 8, "lane = panel column; four rows x eight columns per warp pass");
-    const int rsub = lane / SB, col = lane % SB, lbase = lane - col;
+    constexpr int NW = INVB2_NT / 32, SB = INVB_SB;
+    static_assert(INVB_NB == 32 && SB == 8, "lane = (row group, column pair) of an eight-column sub-panel");
     bool bad = false;
     for (int s0 = 0; s0 < nb && !bad; s0 += SB) {
       const int sb = min(SB, nb - s0);
@@ -200,48 +199,54 @@ __global__ void __launch_bounds__(INVB2_NT, 2) invert_blocked2_kernel(CrowdDev d
         }
         if (tid == 0) piv[c] = p;
         if (!(bv > 0.0) || !isfinite(bv)) { bad = true; break; }   // uniform over the CTA
-        const double prow = XG[p * INVB2_XS + s0 + col], crow = XG[c * INVB2_XS + s0 + col];
-        const double pv = __shfl_sync(0xffffffffu, prow, lbase + jl);
-        const double rc = ((col == jl) ? 1.0 : prow) / pv;   // a true division (see above), one per lane
+        // lane = (row group rg, column pair cp): the lane owns columns 2 cp, 2 cp + 1 of its rows as one 16-byte piece, so
+        // a row costs one shared-memory load, ONE broadcast of its multiplier and one store per lane (with one column per
+        // lane it was twice that; the update loop with its loads, broadcasts and stores is nearly all of a pivot step's
+        // 3.8 k cycles).  The lanes of a quarter-warp take rows r and r + 4 (row stride 34 doubles: 64 bytes apart in the
+        // banks), so the 16-byte accesses are conflict-free.
+        const int cp = lane & 3, rg = lane >> 2, cbase = lane - cp;
+        const double2 prow = *reinterpret_cast<const double2*>(XG + p * INVB2_XS + s0 + 2 * cp);
+        const double2 crow = *reinterpret_cast<const double2*>(XG + c * INVB2_XS + s0 + 2 * cp);
+        const double pv = __shfl_sync(0xffffffffu, (jl & 1) ? prow.y : prow.x, cbase + (jl >> 1));
+        // true divisions (see above), two per lane
+        const double2 rc = make_double2(((2 * cp == jl) ? 1.0 : prow.x) / pv, ((2 * cp + 1 == jl) ? 1.0 : prow.y) / pv);
         __syncthreads();   // rows c and p are in registers everywhere; the partial maxima have been read
         double best = -1.0;
         int bi = c + 1;
-        // a warp pass takes 16 consecutive rows: lane group rsub the rows 4 rsub + i, i = 0..3 in turn.  Rows four apart
-        // sit 8 double-banks apart (row stride 34), so the four groups' 8-column runs tile the 16 double-banks exactly
-        // twice -- two wavefronts per access, the minimum (four with adjacent rows).
-        for (int rb = warp * 4 * RPW; rb < n; rb += 4 * RPW * NW) {   // warp-uniform trip count; four independent rows
-          const int r0 = rb + 4 * rsub;
-          double v[4];
+        const bool next_y = (jl + 1) & 1;   // component of column jl + 1 in the lanes cp == (jl + 1) / 2
+        for (int rb = warp * 16; rb < n; rb += 16 * NW) {   // warp-uniform trip count; a warp pass takes 16 consecutive rows
+          const int r0 = rb + (rg >> 1) + 4 * (rg & 1);
+          double2 v[2];
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int r = r0 + i;
-            v[i] = (r < n) ? XG[r * INVB2_XS + s0 + col] : 0.0;
-            v[i] = (r == p) ? crow : v[i];   // row p receives the old row c
+          for (int i = 0; i < 2; ++i) {
+            const int r = r0 + 8 * i;
+            v[i] = (r < n) ? *reinterpret_cast<const double2*>(XG + r * INVB2_XS + s0 + 2 * cp) : make_double2(0.0, 0.0);
+            if (r == p) v[i] = crow;   // row p receives the old row c
           }
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int r = r0 + i;
-            const double cf = __shfl_sync(0xffffffffu, v[i], lbase + jl);
-            double nv = fma(-cf, rc, (col == jl) ? 0.0 : v[i]);
-            nv = (r == c) ? rc : nv;
-            if (r < n) XG[r * INVB2_XS + s0 + col] = nv;
-            double a = fabs(nv);
+          for (int i = 0; i < 2; ++i) {
+            const int r = r0 + 8 * i;
+            const double cf = __shfl_sync(0xffffffffu, (jl & 1) ? v[i].y : v[i].x, cbase + (jl >> 1));
+            double2 nv = make_double2(fma(-cf, rc.x, (2 * cp == jl) ? 0.0 : v[i].x), fma(-cf, rc.y, (2 * cp + 1 == jl) ? 0.0 : v[i].y));
+            if (r == c) nv = rc;
+            if (r < n) *reinterpret_cast<double2*>(XG + r * INVB2_XS + s0 + 2 * cp) = nv;
+            double a = fabs(next_y ? nv.y : nv.x);
             a = (a == a) ? a : INFINITY;
             const bool take = r > c && r < n && (a > best || (a == best && r < bi));
             best = take ? a : best;
             bi = take ? r : bi;
           }
         }
-        if (jl + 1 < sb) {   // column jl + 1 lives in the lanes col == jl + 1 of the RPW row groups
-          double bj = __shfl_sync(0xffffffffu, best, lbase + jl + 1);
-          int ij = __shfl_sync(0xffffffffu, bi, lbase + jl + 1);
+        if (jl + 1 < sb) {   // column jl + 1 lives in the lanes cp == (jl + 1) / 2 of the eight row groups
+          double bj = best;
+          int ij = bi;
 #pragma unroll
-          for (int o = SB; o < 32; o <<= 1) {
+          for (int o = 4; o < 32; o <<= 1) {
             const double ov = __shfl_xor_sync(0xffffffffu, bj, o);
             const int oi = __shfl_xor_sync(0xffffffffu, ij, o);
             if (ov > bj || (ov == bj && oi < ij)) { bj = ov; ij = oi; }
           }
-          if (lane == 0) { redv[warp] = bj; redi[warp] = ij; }
+          if (lane == ((jl + 1) >> 1)) { redv[warp] = bj; redi[warp] = ij; }
         }
       }
       if (bad) break;
