@@ -79,3 +79,16 @@ def test_null_handles_are_errors_not_crashes():
     assert lib.qmc_crowd_destroy(None) == q.QMC_OK
     out = C.c_void_p()
     assert lib.qmc_crowd_create(None, None, C.byref(out)) == q.QMC_ERR_INVALID_ARG
+
+
+def test_binding_constants_match_the_header():
+    """Option numbers, status codes and the static scratch size are typed twice (header and binding): keep them equal."""
+    txt = (ROOT / "include" / "qmc_crowd.h").read_text()
+    for name in ("QMC_OPT_GRAPH", "QMC_OPT_PROFILE", "QMC_OPT_SUBCROWDS", "QMC_OPT_RECOMPUTE_EVERY", "QMC_OPT_STRIP_ROWS"):
+        m = re.search(rf"#define\s+{name}\s+(\d+)", txt)
+        assert m and int(m.group(1)) == getattr(q, name), name
+    m = re.search(r"#define\s+QMC_STATIC_SCRATCH_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", txt)
+    assert m and (int(m.group(1)) << int(m.group(2))) == q.STATIC_SCRATCH_BYTES
+    for name in ("QMC_OK", "QMC_ERR_INVALID_ARG", "QMC_ERR_CUDA", "QMC_ERR_WORKSPACE", "QMC_ERR_SINGULAR", "QMC_ERR_STATE"):
+        m = re.search(rf"\b{name}\s*=\s*(\d+)", txt)
+        assert m and int(m.group(1)) == getattr(q, name), name
